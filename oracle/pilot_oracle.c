@@ -354,7 +354,11 @@ int pilot_oracle_range(const pilot_refine_inputs* in, const pilot_refine_params*
 static void add_outer(double H[36], double g[6], const double J[6], double r, double wgt) {
   for (int a = 0; a < 6; ++a) {
     g[a] += wgt * J[a] * r;
-    for (int b = 0; b < 6; ++b) H[6 * a + b] += wgt * J[a] * J[b];
+    for (int b = a; b < 6; ++b) {                    /* upper triangle, mirrored: H = H^T exactly */
+      double h = wgt * J[a] * J[b];
+      H[6 * a + b] += h;
+      if (b != a) H[6 * b + a] += h;
+    }
   }
 }
 
@@ -392,8 +396,11 @@ void pilot_oracle_eval(const pilot_refine_config* cfg, const pilot_refine_inputs
         gj[a] = omega * (Ju[a] * b1 + Jv[a] * b2);
         g[a] += gj[a];
         n2 += gj[a] * gj[a];
-        for (int b = 0; b < 6; ++b)
-          H[6 * a + b] += omega * (A11 * Ju[a] * Ju[b] + A12 * (Ju[a] * Jv[b] + Jv[a] * Ju[b]) + A22 * Jv[a] * Jv[b]);
+        for (int b = a; b < 6; ++b) {                /* upper triangle, mirrored: H = H^T exactly */
+          double h = omega * (A11 * Ju[a] * Ju[b] + A12 * (Ju[a] * Jv[b] + Jv[a] * Ju[b]) + A22 * Jv[a] * Jv[b]);
+          H[6 * a + b] += h;
+          if (b != a) H[6 * b + a] += h;
+        }
       }
       gabs += sqrt(n2);
       cost += rho;

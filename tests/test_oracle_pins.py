@@ -1,0 +1,529 @@
+"""Pins for the CPU oracle against what the paper and the mathematics fix (SURVEY.md §8(c) pins 1-11).
+
+The paper prints no worked numeric example for this path (tests/golden/README.md), so every pin is a
+closed form, a finite difference, a library routine, brute force on tiny inputs, or an invariance.
+CPU only (-m "not gpu").
+"""
+import numpy as np
+import pytest
+from scipy.linalg import expm
+from scipy.spatial.transform import Rotation
+
+from oracle import pilot_oracle as po
+from tests.small_problems import tiny
+
+
+def hat(a):
+    return np.array([[0, -a[2], a[1]], [a[2], 0, -a[0]], [-a[1], a[0], 0.0]])
+
+
+def xi_mat(xi):
+    M = np.zeros((4, 4))
+    M[:3, :3] = hat(xi[3:])
+    M[:3, 3] = xi[:3]
+    return M
+
+
+def RC(prob, m=0):
+    return po.pose_to_RC(prob["init_poses"][m])
+
+
+# ------------------------------------------------------------------ pin 8: robust losses
+
+@pytest.mark.parametrize("kind", ["l2", "huber", "cauchy"])
+def test_loss_derivative_matches_fd(kind):
+    for x in [1e-4, 0.003, 0.0099, 0.0101, 0.5, 7.0]:
+        r, d = po.loss(kind, x, 0.1)
+        h = 1e-7 * max(x, 1e-3)
+        fd = (po.loss(kind, x + h, 0.1)[0] - po.loss(kind, x - h, 0.1)[0]) / (2 * h)
+        assert abs(fd - d) <= 1e-5 * max(1.0, abs(d)), (kind, x, fd, d)
+
+
+def test_loss_closed_forms():
+    # Huber on x = squared norm, delta = 0.1: quadratic branch rho = x, linear branch 2 d sqrt(x) - d^2
+    assert po.loss("huber", 0.0025, 0.1) == (0.0025, 1.0)
+    r, d = po.loss("huber", 0.04, 0.1)
+    assert r == pytest.approx(2 * 0.1 * 0.2 - 0.01) and d == pytest.approx(0.5)
+    # C1 at x = delta^2
+    lo, hi = po.loss("huber", 0.01 - 1e-12, 0.1), po.loss("huber", 0.01 + 1e-12, 0.1)
+    assert abs(lo[0] - hi[0]) < 1e-10 and abs(lo[1] - hi[1]) < 1e-9
+    # Cauchy: d^2 ln(1 + x/d^2); -> L2 as the scale grows; scale 0 means L2
+    r, d = po.loss("cauchy", 0.03, 0.1)
+    assert r == pytest.approx(0.01 * np.log(4.0)) and d == pytest.approx(0.25)
+    r, d = po.loss("cauchy", 0.03, 1e6)
+    assert r == pytest.approx(0.03, rel=1e-9) and d == pytest.approx(1.0, rel=1e-9)
+    assert po.loss("cauchy", 0.03, 0.0) == (0.03, 1.0)
+
+
+# ------------------------------------------------------------------ pin 6: SE(3) exp
+
+def test_se3_exp_matches_matrix_exponential():
+    rng = np.random.default_rng(1)
+    for scale in [1e-7, 1e-5, 1e-3, 0.3, 2.5]:
+        xi = rng.normal(size=6) * scale
+        E, V = po.se3_exp(xi)
+        M = expm(xi_mat(xi))                                   # textbook 4x4 matrix exponential
+        assert np.allclose(E, M[:3, :3], atol=1e-13)
+        assert np.allclose(V @ xi[:3], M[:3, 3], atol=1e-13 * max(1, scale))
+        assert np.allclose(E.T @ E, np.eye(3), atol=1e-13) and np.linalg.det(E) == pytest.approx(1.0)
+        assert np.allclose(E, Rotation.from_rotvec(xi[3:]).as_matrix(), atol=1e-13)
+    xi = rng.normal(size=6) * 0.2
+    E1, V1 = po.se3_exp(xi)
+    E2, V2 = po.se3_exp(-xi)
+    assert np.allclose(E1 @ E2, np.eye(3), atol=1e-14)
+    assert np.allclose(E1 @ (V2 @ -xi[:3]) + V1 @ xi[:3], 0, atol=1e-14)   # exp(xi) exp(-xi) = I
+
+
+def test_retract_is_left_multiplication_of_T_cw():
+    rng = np.random.default_rng(2)
+    R = Rotation.from_rotvec(rng.normal(size=3)).as_matrix()
+    Cc = rng.normal(size=3) * 50
+    xi = rng.normal(size=6) * np.array([2, 2, 2, 0.1, 0.1, 0.1])
+    Rn, Cn = po.retract(R, Cc, xi)
+    T = np.eye(4); T[:3, :3] = R; T[:3, 3] = -R @ Cc
+    Tn = expm(xi_mat(xi)) @ T                                  # Eq.(9): T <- exp(xi) T   (reading A1: T = T_cw)
+    assert np.allclose(Rn.reshape(3, 3), Tn[:3, :3], atol=1e-12)
+    assert np.allclose(Cn, -Tn[:3, :3].T @ Tn[:3, 3], atol=1e-10)
+    R0, C0 = po.retract(R, Cc, np.zeros(6))
+    assert np.array_equal(R0.reshape(3, 3), R) and np.array_equal(C0, Cc)
+
+
+# ------------------------------------------------------------------ pin 7: 6x6 solve
+
+def test_chol_solve_matches_numpy():
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        A = rng.normal(size=(9, 6)); A = A.T @ A + 1e-3 * np.eye(6)
+        b = rng.normal(size=6)
+        ok, x = po.chol_solve6(A, b)
+        assert ok and np.allclose(x, np.linalg.solve(A, b), rtol=1e-9, atol=1e-12)
+    ok, _ = po.chol_solve6(-np.eye(6), np.ones(6))
+    assert not ok
+    A = np.eye(6); A[5, 5] = 0.0
+    assert not po.chol_solve6(A, np.ones(6))[0]
+    A = np.eye(6); A[2, 2] = np.nan
+    assert not po.chol_solve6(A, np.ones(6))[0]
+
+
+# ------------------------------------------------------------------ projection + bilinear: closed form on an affine field
+
+def test_photo_point_closed_form_on_affine_field():
+    """Bilinear interpolation reproduces an affine field exactly, so f(u,v) = a + b u + d v with (u,v) from an
+    independent pinhole projection written here; gx = b, gy = d; Juv by finite differences of that projection."""
+    prob = tiny(seed=4, N=20, C=4, affine=True)
+    b = po.Bound(prob)
+    a_, b_, d_ = prob["affine"]
+    fx, fy, cx, cy = prob["K"]
+    T = prob["gt_pose"].reshape(3, 4)
+    R_wc, Cc = T[:, :3], T[:, 3]
+    R, Cv = po.pose_to_RC(T)
+    seen = 0
+    for j in range(20):
+        P = prob["points"][0][j, :3].astype(np.float64)
+        pc = R_wc.T @ (P - Cc)
+        u, v = fx * pc[0] / pc[2] + cx, fy * pc[1] / pc[2] + cy
+        out = po.photo_point(b, 0, R, Cv, j)
+        inside = (0 <= np.floor(u) and np.floor(u) + 1 <= 39 and 0 <= np.floor(v) and np.floor(v) + 1 <= 29)
+        assert (out is not None) == bool(inside and pc[2] > 0.1)
+        if out is None:
+            continue
+        seen += 1
+        assert np.allclose(out["uv"], [u, v], atol=1e-11)
+        f = a_ + b_ * u + d_ * v
+        ref = prob["ref_feat"][0][j].astype(np.float64)
+        # the map is stored in fp32, so the affine field is exact to fp32 rounding of its samples
+        assert np.allclose(out["f"], f, atol=3e-6)
+        assert np.allclose(out["gx"], b_, atol=3e-6) and np.allclose(out["gy"], d_, atol=3e-6)
+        assert np.allclose(out["r"], out["f"] - ref, atol=1e-14)
+        assert out["w"] == 1.0
+    assert seen >= 10
+
+
+def test_visibility_rules():
+    prob = tiny(seed=5, N=6, C=2)
+    T = prob["gt_pose"].reshape(3, 4)
+    fx, fy, cx, cy = prob["K"]
+
+    def world(u, v, Z):  # a point that projects to (u, v) at depth Z
+        pc = np.array([(u - cx) / fx * Z, (v - cy) / fy * Z, Z])
+        return T[:, :3] @ pc + T[:, 3]
+    cases = [((5.5, 5.5, 50.0), True), ((0.01, 0.01, 50.0), True), ((38.99, 28.99, 50.0), True),
+             ((39.01, 10.0, 50.0), False), ((10.0, 29.01, 50.0), False), ((-0.01, 5.0, 50.0), False),
+             ((5.0, 5.0, 0.05), False), ((5.0, 5.0, -10.0), False)]
+    pts = np.array([list(world(*c[0])) + [1.0] for c in cases], np.float32)
+    prob["points"] = [pts]
+    prob["ref_feat"] = [np.zeros((len(cases), 2), np.float32)]
+    # fp32 storage of the points moves u,v by ~1e-5 px: the cases stay 0.01 px away from the border
+    b = po.Bound(prob)
+    R, Cv = po.pose_to_RC(T)
+    got = [po.photo_point(b, 0, R, Cv, j) is not None for j in range(len(cases))]
+    want = [c[1] for c in cases]
+    for j, (g, w) in enumerate(zip(got, want)):
+        assert g == w, (j, cases[j])
+
+
+# ------------------------------------------------------------------ pin 2: finite-difference Jacobians
+
+def perturbed(R, Cv, i, eps):
+    xi = np.zeros(6); xi[i] = eps
+    return po.retract(R, Cv, xi)
+
+
+def test_photo_jacobian_matches_finite_differences():
+    prob = tiny(seed=6, N=30, C=3, conf=False)
+    b = po.Bound(prob)
+    R, Cv = RC(prob)
+    eps, checked = 1e-6, 0
+    for j in range(30):
+        o = po.photo_point(b, 0, R, Cv, j)
+        if o is None:
+            continue
+        fr = o["uv"] - np.floor(o["uv"])
+        if fr.min() < 0.05 or fr.max() > 0.95:
+            continue                                           # keep the stencil inside one bilinear cell
+        G = np.stack([o["gx"], o["gy"]], 1)                    # C x 2
+        J = G @ o["Juv"]                                       # C x 6 = dr/dxi
+        for i in range(6):
+            rp = po.photo_point(b, 0, *perturbed(R, Cv, i, eps), j)
+            rm = po.photo_point(b, 0, *perturbed(R, Cv, i, -eps), j)
+            fd = (rp["r"] - rm["r"]) / (2 * eps)
+            assert np.allclose(fd, J[:, i], rtol=2e-6, atol=1e-7 * np.abs(J).max()), (j, i)
+            fd_uv = (rp["uv"] - rm["uv"]) / (2 * eps)
+            assert np.allclose(fd_uv, o["Juv"][:, i], rtol=1e-6, atol=1e-6)
+        checked += 1
+    assert checked >= 8
+
+
+def test_gravity_jacobian_and_closed_form():
+    prob = tiny(seed=7)
+    b = po.Bound(prob)
+    R, Cv = RC(prob)
+    r, J = po.gravity(b, R)
+    for i in range(6):
+        rp, _ = po.gravity(b, perturbed(R, Cv, i, 1e-6)[0])
+        rm, _ = po.gravity(b, perturbed(R, Cv, i, -1e-6)[0])
+        assert np.allclose((rp - rm) / 2e-6, J[:, i], atol=1e-9)
+    # closed form: |r|^2 = 2 (1 - cos theta) for a tilt theta between predicted and measured gravity
+    e = R.reshape(3, 3) @ prob["gravity_world"]
+    for theta in [0.0, 0.01, 0.3]:
+        axis = np.cross(e, [1.0, 0.2, 0.1]); axis /= np.linalg.norm(axis)
+        prob2 = dict(prob); prob2["gravity_imu"] = Rotation.from_rotvec(axis * theta).as_matrix() @ e
+        r2, _ = po.gravity(po.Bound(prob2), R)
+        assert r2 @ r2 == pytest.approx(2 * (1 - np.cos(theta)), abs=5e-7 * theta + 1e-13)  # gamma^imu is an fp32 input
+    # yaw (rotation about gamma^W in the world) is unobservable: PAPER.md:392
+    prob3 = dict(prob); prob3["gravity_imu"] = e
+    b3 = po.Bound(prob3)
+    Ryaw = R.reshape(3, 3) @ Rotation.from_rotvec(np.array([0, 0, 1.0]) * 0.7).as_matrix().T
+    assert np.allclose(po.gravity(b3, Ryaw)[0], 0, atol=1e-7)   # gravity_imu passes through fp32
+    # H_grav has rank 2; null space = translations + phi || e
+    par = dict(w_gravity=1.0, gravity_scale=0.0, range_mode="off")
+    ev = po.evaluate(po.Bound(prob, par), 0, R, Cv, which=2)
+    s = np.linalg.svd(ev["H"], compute_uv=False)
+    assert s[1] > 0.5 and s[2] < 1e-12
+    null = np.zeros(6); null[3:] = e
+    assert np.allclose(ev["H"] @ null, 0, atol=1e-12)
+    assert np.allclose(ev["H"][:3], 0)
+
+
+@pytest.mark.parametrize("mode", ["height", "march"])
+def test_range_jacobian_matches_finite_differences(mode):
+    prob = tiny(seed=8, n_hyp=2)
+    prob["range_meas"] = 79.0
+    b = po.Bound(prob, dict(range_mode=mode, bisect_steps=40))
+    R, Cv = RC(prob, 1)      # the perturbed pose: the unperturbed centre ray lands exactly on a DSM cell edge (a kink)
+    out = po.range_term(b, R, Cv)
+    assert out is not None
+    r, J, dh = out
+    for i in range(6):
+        eps = 1e-5
+        rp = po.range_term(b, *perturbed(R, Cv, i, eps))[0]
+        rm = po.range_term(b, *perturbed(R, Cv, i, -eps))[0]
+        assert (rp - rm) / (2 * eps) == pytest.approx(J[i], rel=2e-5, abs=2e-6), (mode, i)
+
+
+# ------------------------------------------------------------------ pin 5: range closed forms on a plane
+
+def test_range_closed_form_on_plane():
+    h0, pa, pb = 4.0, 0.03, -0.05
+    prob = tiny(seed=9, dsm_plane=(h0, pa, pb))
+    R, Cv = RC(prob)
+    n = np.array([-pa, -pb, 1.0])
+    w = R.reshape(3, 3).T @ prob["range_ray_cam"]
+    d_hit = -(n @ Cv - h0) / (n @ w)
+    for dm in [70.0, d_hit, 95.0]:
+        prob["range_meas"] = dm
+        bh = po.Bound(prob, dict(range_mode="height"))
+        bm = po.Bound(prob, dict(range_mode="march"))
+        dmf = float(np.float32(dm))
+        rh = po.range_term(bh, R, Cv)[0]
+        rm, _, dh = po.range_term(bm, R, Cv)
+        assert rh == pytest.approx(n @ (Cv + dmf * w) - h0, abs=2e-5)       # Eq.(5)-(6); the DSM is fp32
+        assert dh == pytest.approx(d_hit, abs=2e-5)                          # secant is exact on a plane
+        assert rm == pytest.approx(d_hit - dmf, abs=2e-5)
+        assert rh == pytest.approx((n @ w) * (dmf - dh), abs=2e-5)
+    # a ray that never meets the surface within t_far, or leaves the map, is skipped
+    prob["range_meas"] = 10.0
+    assert po.range_term(po.Bound(prob, dict(range_mode="march")), R, Cv) is None
+    up = R.reshape(3, 3).copy(); up[2] = -up[2]; up[1] = -up[1]              # look away from the ground
+    assert po.range_term(po.Bound(prob, dict(range_mode="height")), up, Cv) is None
+
+
+def test_dsm_sample_on_plane_and_bounds():
+    prob = tiny(seed=10, dsm_plane=(2.0, 0.1, -0.2))
+    b = po.Bound(prob)
+    ok, z, dx, dy = po.dsm_sample(b, 3.3, -7.7)
+    assert ok and z == pytest.approx(2.0 + 0.33 + 1.54, abs=1e-5)
+    assert dx == pytest.approx(0.1, abs=1e-6) and dy == pytest.approx(-0.2, abs=1e-6)
+    assert po.dsm_sample(b, -32.0, -32.0)[0] and po.dsm_sample(b, 31.99, 31.99)[0]
+    assert not po.dsm_sample(b, 32.0, 0.0)[0] and not po.dsm_sample(b, 0.0, -32.01)[0]
+    assert not po.dsm_sample(b, float("nan"), 0.0)[0]
+
+
+# ------------------------------------------------------------------ pins 3, 11: H = J^T J brute force, symmetric PSD, gradient of the cost
+
+def stacked(b, prob, R, Cv):
+    rows, res = [], []
+    for j in range(prob["points"][0].shape[0]):
+        o = po.photo_point(b, 0, R, Cv, j)
+        if o is None:
+            continue
+        rows.append(np.sqrt(o["w"]) * np.stack([o["gx"], o["gy"]], 1) @ o["Juv"])
+        res.append(np.sqrt(o["w"]) * o["r"])
+    return np.concatenate(rows, 0), np.concatenate(res, 0)
+
+
+def test_brute_force_normal_equations_l2():
+    prob = tiny(seed=11, N=8, C=4, conf=True)
+    b = po.Bound(prob, dict(loss="l2", w_gravity=0.0, range_mode="off"))
+    R, Cv = RC(prob)
+    J, r = stacked(b, prob, R, Cv)
+    ev = po.evaluate(b, 0, R, Cv)
+    assert ev["n_valid"] == J.shape[0] // 4 and ev["n_valid"] >= 5
+    assert np.allclose(ev["H"], J.T @ J, rtol=1e-12, atol=1e-12 * np.abs(J.T @ J).max())
+    assert np.allclose(ev["g"], J.T @ r, rtol=1e-12, atol=1e-12 * np.abs(J.T @ r).max())
+    assert ev["cost"] == pytest.approx(r @ r, rel=1e-13)
+    assert np.array_equal(ev["H"], ev["H"].T)
+    assert np.linalg.eigvalsh(ev["H"]).min() >= -1e-12 * np.trace(ev["H"])
+
+
+def test_single_point_single_channel_rank_one():
+    prob = tiny(seed=12, N=1, C=1)
+    prob["points"][0][0, :3] = [1.0, 2.0, 5.0]
+    b = po.Bound(prob)
+    ev = po.evaluate(b, 0, *RC(prob))
+    assert ev["n_valid"] == 1
+    s = np.linalg.svd(ev["H"], compute_uv=False)
+    assert s[0] > 0 and s[1] < 1e-12 * s[0]
+
+
+@pytest.mark.parametrize("loss", ["l2", "huber", "cauchy"])
+def test_cost_gradient_is_2g(loss):
+    prob = tiny(seed=13, N=40, C=3, conf=True, n_hyp=2)
+    prob["query_conf"] = [None]    # reading A5: w^q is held constant in the linearisation, so only w_ref here
+    prob["range_meas"] = 79.0
+    par = dict(loss=loss, loss_scale=0.3, w_gravity=0.7, gravity_scale=0.05, range_mode="march", w_range=0.02,
+               range_scale=0.5, bisect_steps=40)
+    b = po.Bound(prob, par)
+    R, Cv = RC(prob, 1)
+    ev = po.evaluate(b, 0, R, Cv)
+    assert ev["flags"] == 0
+    for i in range(6):
+        eps = 1e-6
+        cp = po.evaluate(b, 0, *perturbed(R, Cv, i, eps))["cost"]
+        cm = po.evaluate(b, 0, *perturbed(R, Cv, i, -eps))["cost"]
+        assert (cp - cm) / (2 * eps) == pytest.approx(2 * ev["g"][i], rel=3e-5, abs=1e-6 * np.abs(ev["g"]).max())
+    assert np.array_equal(ev["H"], ev["H"].T)
+    assert np.linalg.eigvalsh(ev["H"]).min() >= -1e-12 * np.trace(ev["H"])
+
+
+def test_robust_weight_and_confidence():
+    """omega = w rho'(w s) (reading A4/A5): compare with the L2 system of one point rescaled by hand."""
+    prob = tiny(seed=14, N=1, C=3, conf=True)
+    prob["points"][0][0, :3] = [1.0, 2.0, 5.0]
+    R, Cv = RC(prob)
+    b2 = po.Bound(prob, dict(loss="l2"))
+    o = po.photo_point(b2, 0, R, Cv, 0)
+    s, w = o["r"] @ o["r"], o["w"]
+    assert w != 1.0
+    e2 = po.evaluate(b2, 0, R, Cv)
+    for loss, scale in [("huber", 0.05), ("cauchy", 0.2)]:
+        ev = po.evaluate(po.Bound(prob, dict(loss=loss, loss_scale=scale)), 0, R, Cv)
+        rho, drho = po.loss(loss, w * s, float(np.float32(scale)))   # the scale is an fp32 field of the params struct
+        assert drho < 1.0
+        assert np.allclose(ev["H"], e2["H"] * drho, rtol=1e-12, atol=1e-13 * np.abs(e2["H"]).max())
+        assert np.allclose(ev["g"], e2["g"] * drho, rtol=1e-12, atol=1e-13 * np.abs(e2["g"]).max())
+        assert ev["cost"] == pytest.approx(rho, rel=1e-13)
+
+
+# ------------------------------------------------------------------ pin 1: zero residual / gradient / step at the generating pose
+
+def test_zero_at_generating_pose():
+    prob = tiny(seed=15, N=40, C=4, affine=True)
+    a_, b_, d_ = prob["affine"]
+    fx, fy, cx, cy = prob["K"]
+    T = prob["gt_pose"].reshape(3, 4)
+    P = prob["points"][0][:, :3].astype(np.float64)
+    pc = (P - T[:, 3]) @ T[:, :3]
+    u, v = fx * pc[:, 0] / pc[:, 2] + cx, fy * pc[:, 1] / pc[:, 2] + cy
+    prob["ref_feat"] = [(a_ + b_ * u[:, None] + d_ * v[:, None]).astype(np.float32)]   # closed form, sigma = 0
+    prob["params"] = dict(iters=[4], loss="l2", min_valid=1)
+    b = po.Bound(prob)
+    R, Cv = RC(prob)
+    ev = po.evaluate(b, 0, R, Cv)
+    assert ev["n_valid"] >= 20
+    # everything is exact up to the fp32 storage of the map and the reference features (~1e-7 relative)
+    assert ev["cost"] < 1e-10
+    # Cauchy-Schwarz: |g_i| = |sum J_i r| <= sqrt(H_ii cost) -> the gradient vanishes with the residual
+    assert np.all(np.abs(ev["g"]) <= np.sqrt(np.diag(ev["H"]) * ev["cost"]) * (1 + 1e-9))
+    o = po.run(b)
+    Tn = o["poses64"][0].reshape(3, 4)
+    assert np.linalg.norm(Tn[:, 3] - T[:, 3]) < 1e-3 and np.allclose(Tn[:, :3], T[:, :3], atol=1e-5)
+    assert o["cost64"][0] <= ev["cost"]
+
+
+# ------------------------------------------------------------------ pin 10: invariances
+
+def test_permutation_and_duplication():
+    prob = tiny(seed=16, N=50, C=3, conf=True)
+    par = dict(loss="cauchy", loss_scale=0.3)
+    R, Cv = RC(prob)
+    e0 = po.evaluate(po.Bound(prob, par), 0, R, Cv)
+    perm = np.random.default_rng(0).permutation(50)
+    p2 = dict(prob); p2["points"] = [prob["points"][0][perm]]; p2["ref_feat"] = [prob["ref_feat"][0][perm]]
+    e1 = po.evaluate(po.Bound(p2, par), 0, R, Cv)
+    assert np.allclose(e0["H"], e1["H"], rtol=1e-12, atol=1e-12 * np.abs(e0["H"]).max())
+    assert np.allclose(e0["g"], e1["g"], rtol=1e-12, atol=1e-12 * e0["g_abs"]) and e0["n_valid"] == e1["n_valid"]
+    p3 = dict(prob); p3["points"] = [np.tile(prob["points"][0], (2, 1))]; p3["ref_feat"] = [np.tile(prob["ref_feat"][0], (2, 1))]
+    e2 = po.evaluate(po.Bound(p3, par), 0, R, Cv)
+    assert np.allclose(e2["H"], 2 * e0["H"], rtol=1e-12, atol=1e-12 * np.abs(e0["H"]).max())
+    assert np.allclose(e2["g"], 2 * e0["g"], rtol=1e-12, atol=1e-12 * e0["g_abs"])
+    assert e2["cost"] == pytest.approx(2 * e0["cost"], rel=1e-13) and e2["n_valid"] == 2 * e0["n_valid"]
+
+
+FULL = dict(iters=[4], loss="huber", loss_scale=0.3, w_gravity=1.0, gravity_scale=0.1, range_mode="march",
+            w_range=0.05, range_scale=5.0, min_valid=4)
+
+
+def test_batch_equals_single_runs_and_subset_selection():
+    prob = tiny(seed=17, N=60, C=3, n_hyp=4)
+    prob["range_meas"] = 79.0
+    prob["params"] = FULL
+    o = po.run(po.Bound(prob), n_threads=4)
+    for m in range(4):
+        p1 = dict(prob); p1["init_poses"] = prob["init_poses"][m:m + 1]
+        o1 = po.run(po.Bound(p1))
+        assert np.array_equal(o1["poses64"][0], o["poses64"][m])
+        assert np.array_equal(o1["iter_hessian"][:, 0], o["iter_hessian"][:, m])
+        assert np.array_equal(o1["iter_lambda"][:, 0], o["iter_lambda"][:, m])
+    sub = po.run(po.Bound(prob), hyp_begin=1, hyp_step=2)
+    assert np.array_equal(sub["poses64"][1], o["poses64"][1]) and np.array_equal(sub["poses64"][3], o["poses64"][3])
+    assert not sub["poses64"][0].any() and not sub["poses64"][2].any()
+
+
+def test_world_origin_shift_invariance():
+    """Pins reading A1 (Eq.9 acts on T_cw): shifting every P, C and the DSM origin changes nothing."""
+    sh = (256.0, -512.0, 64.0)     # exactly representable, so fp32 inputs shift without rounding
+    pa = tiny(seed=18, N=60, C=3, n_hyp=2)
+    pb = tiny(seed=18, N=60, C=3, n_hyp=2, origin_shift=sh)
+    for p in (pa, pb):
+        p["range_meas"] = 79.0
+        p["params"] = FULL
+    oa, ob = po.run(po.Bound(pa)), po.run(po.Bound(pb))
+    assert np.allclose(oa["iter_hessian"], ob["iter_hessian"], rtol=1e-4, atol=1e-4 * np.abs(oa["iter_hessian"]).max())
+    assert np.allclose(oa["iter_cost"], ob["iter_cost"], rtol=1e-5)
+    Ta, Tb = oa["poses64"].reshape(2, 3, 4), ob["poses64"].reshape(2, 3, 4)
+    assert np.allclose(Ta[:, :, :3], Tb[:, :, :3], atol=1e-5)
+    assert np.allclose(Ta[:, :, 3] + np.array(sh), Tb[:, :, 3], atol=1e-3)
+
+
+# ------------------------------------------------------------------ pin 9: LM loop semantics and convergence
+
+def test_lm_records_and_schedule():
+    prob = tiny(seed=19, N=80, C=4, n_hyp=3)
+    prob["params"] = dict(iters=[6], loss="l2", min_valid=4, lambda_init=1e-2)
+    b = po.Bound(prob)
+    o = po.run(b)
+    for m in range(3):
+        R, Cv = RC(prob, m)
+        ev = po.evaluate(b, 0, R, Cv)
+        # record 0 is the system at the input pose, taken before the first solve
+        assert np.allclose(o["iter_hessian"][0, m].reshape(6, 6), ev["H"], rtol=1e-6, atol=1e-6 * np.abs(ev["H"]).max())
+        assert o["iter_cost"][0, m] == pytest.approx(ev["cost"], rel=1e-6)
+        assert np.allclose(o["iter_poses"][0, m], prob["init_poses"][m], atol=1e-7)
+        lam, cost = o["iter_lambda"][:, m], o["iter_cost"][:, m]
+        assert lam[0] == np.float32(1e-2)
+        assert np.all(np.diff(cost) <= 0)                      # adaptive LM never accepts an increase
+        for k in range(5):
+            accepted = cost[k + 1] < cost[k] or not np.array_equal(o["iter_poses"][k + 1, m], o["iter_poses"][k, m])
+            want = max(lam[k] * 0.1, 1e-8) if accepted else min(lam[k] * 10, 1e8)
+            assert lam[k + 1] == pytest.approx(want, rel=1e-6)
+        assert o["cost64"][m] <= cost[-1] + 1e-12
+    # FIXED mode: lambda constant, every step taken
+    of = po.run(po.Bound(prob, dict(lm_mode="fixed")))
+    assert np.all(of["iter_lambda"] == np.float32(1e-2))
+    # iters = {1}: exactly one recorded system, at the input pose
+    o1 = po.run(po.Bound(prob, dict(iters=[1])))
+    assert o1["iter_hessian"].shape[0] == 1 and np.array_equal(o1["iter_hessian"][0], o["iter_hessian"][0])
+
+
+def test_convergence_config0_noise_free():
+    from paper_2606_31098_b200 import workloads as wl
+    prob = wl.config0(noise=0.0)
+    o = po.run(po.Bound(prob, dict(iters=[12])))
+    T, Tg = o["poses64"][0].reshape(3, 4), prob["gt_pose"].reshape(3, 4)
+    ang = np.degrees(np.arccos(np.clip((np.trace(T[:, :3].T @ Tg[:, :3]) - 1) / 2, -1, 1)))
+    # analytic reference vs bilinear map: the residual floor is the interpolation error, not zero
+    assert np.linalg.norm(T[:, 3] - Tg[:, 3]) < 0.1 and ang < 0.05
+    assert np.all(np.diff(o["iter_cost"][:, 0]) <= 0) and o["cost64"][0] < 0.02 * o["iter_cost"][0, 0]
+    assert o["status"][0] == 0
+
+
+def test_min_valid_gives_infinite_cost_and_status():
+    prob = tiny(seed=20, N=10, C=2)
+    prob["params"] = dict(iters=[2], loss="l2", min_valid=11)
+    b = po.Bound(prob)
+    ev = po.evaluate(b, 0, *RC(prob))
+    assert ev["cost"] == np.inf and ev["flags"] & 2
+    o = po.run(b)
+    assert o["status"][0] & 2 and np.isinf(o["cost"][0])
+    assert np.allclose(o["poses"][0], prob["init_poses"][0], atol=1e-6)   # inf never beats inf: all steps rejected
+
+
+# ------------------------------------------------------------------ reading A7: central-difference gradient mode, closed form
+
+def test_central_sampled_gradient_on_quadratic_field():
+    """Central differences are exact on quadratics and bilinear sampling is exact on affine functions, so
+    gx = b + 2 e u + g v and gy = d + 2 f v + g u away from the border."""
+    prob = tiny(seed=21, N=30, C=2)
+    W, H = 40, 30
+    ys, xs = np.mgrid[0:H, 0:W].astype(np.float64)
+    co = np.array([[0.3, 0.05, -0.02, 0.004, -0.003, 0.002], [-0.1, -0.03, 0.04, -0.002, 0.001, 0.003]])
+    F = np.stack([c[0] + c[1] * xs + c[2] * ys + c[3] * xs * xs + c[4] * ys * ys + c[5] * xs * ys for c in co], -1)
+    prob["query_feat"] = [F.astype(np.float32)]
+    b = po.Bound(prob, dict(grad_mode="central_sampled"))
+    R, Cv = RC(prob)
+    n = 0
+    for j in range(30):
+        o = po.photo_point(b, 0, R, Cv, j)
+        if o is None or not (1 <= o["uv"][0] < W - 2 and 1 <= o["uv"][1] < H - 2):
+            continue
+        u, v = o["uv"]
+        assert np.allclose(o["gx"], co[:, 1] + 2 * co[:, 3] * u + co[:, 5] * v, atol=2e-5)
+        assert np.allclose(o["gy"], co[:, 2] + 2 * co[:, 4] * v + co[:, 5] * u, atol=2e-5)
+        n += 1
+    assert n >= 10
+
+
+# ------------------------------------------------------------------ element decoding
+
+@pytest.mark.parametrize("dtype", ["bf16", "f16"])
+def test_half_types_decode_exactly(dtype):
+    import torch
+    pf = tiny(seed=22, N=20, C=4, dtype=dtype)
+    tdt = torch.bfloat16 if dtype == "bf16" else torch.float16
+    q = torch.from_numpy(pf["query_feat"][0].view(np.int16)).view(tdt).float().numpy()     # library decode
+    r = torch.from_numpy(pf["ref_feat"][0].view(np.int16)).view(tdt).float().numpy()
+    p32 = dict(pf); p32["dtype"] = "f32"; p32["query_feat"] = [q]; p32["ref_feat"] = [r]
+    R, Cv = RC(pf)
+    e16, e32 = po.evaluate(po.Bound(pf), 0, R, Cv), po.evaluate(po.Bound(p32), 0, R, Cv)
+    assert np.array_equal(e16["H"], e32["H"]) and np.array_equal(e16["g"], e32["g"]) and e16["cost"] == e32["cost"]
