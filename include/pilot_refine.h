@@ -144,19 +144,26 @@ int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in,
 int pilot_refine_destroy(pilot_refine_handle* h);
 
 /*
- * Host-buffer convenience wrapper (the end-to-end path bench.py's "e2e" times):
- * every "_dev" pointer of `in` and `out` is a HOST pointer here. Copies the
- * inputs to device staging inside the handle's workspace on `cuda_stream`, runs
- * pilot_refine_run, copies the requested outputs back and synchronises the
- * stream before returning. The handle must have been created with
- * pilot_refine_workspace_bytes_host() bytes of scratch (or workspace_dev NULL
- * and `host_staging` != 0 in the call below).
+ * Host-buffer path (what bench.py's "e2e" times): every "_dev" pointer of `in_host` and
+ * `out_host` is a HOST pointer (pinned memory recommended). run_host copies the inputs into
+ * device staging owned by the handle (cudaMemcpyAsync on `cuda_stream`), enqueues
+ * pilot_refine_run, copies the requested outputs back and synchronises the stream before
+ * returning. The staging is sized at create_host() from cfg plus the DSM capacity given
+ * there and is allocated once with cudaMalloc (cfg->workspace_dev must be NULL); a run whose
+ * DSM exceeds that capacity returns PILOT_ERR_UNSUPPORTED.
  */
-size_t pilot_refine_workspace_bytes_host(const pilot_refine_config* cfg);
-int pilot_refine_create_host(const pilot_refine_config* cfg, pilot_refine_handle** out);
+int pilot_refine_create_host(const pilot_refine_config* cfg, int max_dsm_width, int max_dsm_height,
+                             pilot_refine_handle** out);
 int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in_host,
                           const pilot_refine_params* p, const pilot_refine_outputs* out_host,
                           void* cuda_stream);
+
+/*
+ * Tuning knob: anchors per CTA of the photo kernel (a multiple of 256; 0 = built-in heuristic,
+ * which sizes the grid to a few waves of 2 CTAs per SM). Results do not depend on it beyond
+ * fp32 summation order.
+ */
+int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk);
 
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */
 int pilot_refine_last_launches(const pilot_refine_handle* h);

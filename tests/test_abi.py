@@ -1,0 +1,49 @@
+"""The C-ABI library loads and exports every symbol include/pilot_refine.h declares (no compute calls)."""
+import ctypes
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "pilot_refine.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(pilot_refine_[a-z_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2606_31098_b200 import build
+    lib = ctypes.CDLL(build.build())
+    names = declared_functions()
+    assert {"pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_pure_host_entry_points():
+    from paper_2606_31098_b200 import binding
+    L = binding.lib()
+    cfg = binding.Config()
+    assert L.pilot_refine_workspace_bytes(ctypes.byref(cfg)) == 0          # bad config
+    cfg.n_levels, cfg.feat_dtype = 1, 1
+    cfg.width[0], cfg.height[0], cfg.channels[0] = 480, 270, 32
+    cfg.max_hypotheses, cfg.max_points, cfg.max_total_iters = 64, 4096, 30
+    n = L.pilot_refine_workspace_bytes(ctypes.byref(cfg))
+    assert n > 64 * 16 * 128 and n % 256 == 0
+    assert L.pilot_refine_destroy(None) == 0
+    assert L.pilot_refine_last_launches(None) == 0
+    h = ctypes.c_void_p()
+    assert L.pilot_refine_create(None, ctypes.byref(h)) == -1
+    assert L.pilot_refine_run(None, None, None, None, None) == -1
+
+
+def test_binding_refuses_without_gpu():
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2606_31098_b200 import binding
+    from tests.small_problems import tiny
+    with pytest.raises(RuntimeError):
+        binding.refine(tiny())

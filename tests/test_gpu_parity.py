@@ -1,0 +1,165 @@
+"""GPU-vs-oracle parity through the C-ABI (the -m gpu tier). Tolerances are north_star's:
+H, g within 1e-4 relative (fp32 features) / 5e-3 (bf16, f16); refined poses within 1e-3 rad & 1e-3 m (fp32) /
+5e-3 (bf16) for every hypothesis the oracle flags converged."""
+import numpy as np
+import pytest
+
+from paper_2606_31098_b200 import workloads as wl
+from tests import parity
+from tests.small_problems import tiny
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": (1e-4, 1e-3), "bf16": (5e-3, 5e-3), "f16": (5e-3, 5e-3)}
+
+
+def both(prob, params=None):
+    from oracle import pilot_oracle as po
+    from paper_2606_31098_b200 import binding
+    P = dict(prob.get("params", {})); P.update(params or {})
+    gpu = binding.refine(prob, P)
+    orc = po.run(po.Bound(prob, P), n_threads=8)
+    return gpu, orc
+
+
+def check_systems(gpu, orc, dtype, recs=(0,)):
+    tol = TOL[dtype][0]
+    for rec in recs:
+        eH, eg, ec = parity.system_errors(gpu, orc, rec)
+        assert eH.max() <= tol, ("H", rec, eH.max())
+        assert eg.max() <= tol, ("g", rec, eg.max())
+        assert ec.max() <= tol, ("cost", rec, ec.max())
+
+
+def check_poses(gpu, orc, dtype, min_converged=1):
+    tol = TOL[dtype][1]
+    conv = parity.converged(orc)
+    assert conv.sum() >= min_converged, conv.sum()
+    er, et = parity.pose_errors(gpu, orc)
+    assert er[conv].max() <= tol and et[conv].max() <= tol, (er[conv].max(), et[conv].max())
+    best_o, best_g = int(np.argmin(orc["cost64"])), int(np.argmin(gpu["cost"]))
+    assert er[best_o] <= tol and et[best_o] <= tol
+    assert abs(float(gpu["cost"][best_g]) - orc["cost64"][best_o]) <= 1e-3 * abs(orc["cost64"][best_o])
+    return conv
+
+
+def test_config0_fp32():
+    prob = wl.config0()
+    gpu, orc = both(prob)
+    check_systems(gpu, orc, "f32", recs=(0,))
+    assert np.array_equal(gpu["n_valid"], orc["n_valid"])
+    er, et = parity.pose_errors(gpu, orc)
+    assert er.max() <= 1e-3 and et.max() <= 1e-3
+    assert abs(gpu["cost"][0] - orc["cost"][0]) <= 1e-4 * orc["cost"][0]
+    assert gpu["launches"] == 1 + 6
+
+
+def test_config0_converged_pose_fp32():
+    prob = wl.config0()
+    gpu, orc = both(prob, dict(iters=[15]))
+    check_poses(gpu, orc, "f32")
+
+
+def test_config1_full():
+    prob = wl.config1()
+    gpu, orc = both(prob)
+    # record 0 of each level-0 hypothesis: system at the input pose
+    check_systems(gpu, orc, "bf16", recs=(0,))
+    conv = check_poses(gpu, orc, "bf16", min_converged=48)
+    assert np.array_equal(gpu["status"][conv], orc["status"][conv])
+    assert np.abs(gpu["n_valid"][conv] - orc["n_valid"][conv]).max() <= 2
+
+
+@pytest.mark.parametrize("level", [0, 1, 2])
+def test_config1_teacher_forced_every_level(level):
+    """Same poses in both: systems at the oracle's own iterate poses of that level (several tiles, ragged tail)."""
+    from oracle import pilot_oracle as po
+    prob = wl.config1(N=4096 - 37)
+    orc_full = po.run(po.Bound(prob), n_threads=8)
+    rec = 10 * level + 3
+    poses = orc_full["iter_poses"][rec]
+    q = parity.level_slice(prob, level, poses)
+    gpu, orc = both(q)
+    check_systems(gpu, orc, "bf16")
+    assert np.abs(gpu["n_valid"] - orc["n_valid"]).max() <= 1
+
+
+@pytest.mark.parametrize("dtype,C", [("f32", 4), ("f32", 8), ("f32", 32), ("bf16", 8), ("bf16", 16), ("bf16", 128),
+                                      ("f16", 32), ("f16", 64), ("bf16", 256)])
+def test_lane_group_widths(dtype, C):
+    """Every lanes-per-unit variant G = C*s/16 in {1..32}, with reference and query confidence weights."""
+    prob = tiny(seed=30, N=700, C=C, n_hyp=5, dtype=dtype, conf=True, W=64, H=48)
+    prob["range_meas"] = 79.0
+    P = dict(iters=[3], loss="cauchy", loss_scale=0.5, w_gravity=1.0, gravity_scale=0.1, range_mode="height",
+             w_range=0.05, range_scale=5.0, min_valid=4)
+    gpu, orc = both(prob, P)
+    check_systems(gpu, orc, dtype, recs=(0,))
+    assert np.array_equal(gpu["n_valid"], orc["n_valid"])
+
+
+@pytest.mark.parametrize("loss", ["l2", "huber", "cauchy"])
+@pytest.mark.parametrize("rmode", ["off", "height", "march"])
+def test_losses_and_range_modes(loss, rmode):
+    prob = tiny(seed=31, N=300, C=8, n_hyp=4, dtype="f32")
+    prob["range_meas"] = 79.0
+    P = dict(iters=[4], loss=loss, loss_scale=0.3, w_gravity=0.5, gravity_scale=0.05, range_mode=rmode,
+             w_range=0.05, range_scale=0.5, min_valid=4)
+    gpu, orc = both(prob, P)
+    check_systems(gpu, orc, "f32", recs=(0, 1))
+    assert np.allclose(gpu["iter_lambda"], orc["iter_lambda"], rtol=1e-6)
+
+
+def test_lm_modes_and_damping():
+    prob = tiny(seed=32, N=300, C=8, n_hyp=3, dtype="f32")
+    for P in (dict(lm_mode="fixed"), dict(damp_mode="diag"), dict(lm_mode="fixed", damp_mode="diag", lambda_init=1.0)):
+        P = dict(dict(iters=[3], loss="huber", loss_scale=0.3, min_valid=4), **P)
+        gpu, orc = both(prob, P)
+        check_systems(gpu, orc, "f32", recs=(0, 1, 2))
+        er, et = parity.pose_errors(gpu, orc)
+        assert er.max() < 1e-4 and et.max() < 1e-3
+
+
+def test_edge_cases():
+    from paper_2606_31098_b200 import binding
+    # all anchors behind the camera / off the image: n_valid = 0 -> cost inf, status FEW_VALID, pose unchanged
+    prob = tiny(seed=33, N=40, C=4, n_hyp=2)
+    prob["points"][0][:, 2] += 500.0
+    gpu, orc = both(prob, dict(iters=[2], min_valid=1))
+    assert np.all(gpu["n_valid"] == 0) and np.all(np.isinf(gpu["cost"])) and np.all(gpu["status"] & 2)
+    assert np.array_equal(gpu["status"], orc["status"])
+    assert np.allclose(gpu["poses"], prob["init_poses"], atol=1e-6)
+    # zero points, zero iterations
+    prob = tiny(seed=34, N=20, C=4, n_hyp=2)
+    g0 = binding.refine(prob, dict(iters=[0], min_valid=1))
+    assert np.allclose(g0["poses"], prob["init_poses"], atol=1e-6) and g0["launches"] == 2
+    prob["points"] = [np.zeros((0, 4), np.float32)]; prob["ref_feat"] = [np.zeros((0, 4), np.float32)]
+    g1 = binding.refine(prob, dict(iters=[2], min_valid=0, w_gravity=1.0))
+    o1 = __import__("oracle.pilot_oracle", fromlist=["x"])
+    orc = o1.run(o1.Bound(prob, dict(iters=[2], min_valid=0, w_gravity=1.0)))
+    assert np.allclose(g1["poses"], orc["poses"], atol=1e-5)
+    # range prior that cannot be evaluated: status RANGE_SKIP on both sides
+    prob = tiny(seed=35, N=100, C=4, n_hyp=2)
+    prob["range_meas"] = 5.0
+    gpu, orc = both(prob, dict(iters=[2], range_mode="march", min_valid=4))
+    assert np.all(gpu["status"] & 8) and np.array_equal(gpu["status"], orc["status"])
+
+
+def test_run_is_deterministic():
+    from paper_2606_31098_b200 import binding
+    prob = wl.config1(H=16, N=1500, iters=(3, 3, 3))
+    a, b = binding.refine(prob), binding.refine(prob)
+    for k in ("poses", "cost", "iter_hessian", "iter_gradient"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_host_path_matches_device_path():
+    import torch
+    from paper_2606_31098_b200 import binding
+    prob = wl.config1(H=8, N=1000, iters=(2, 2, 2))
+    dev = binding.refine(prob)
+    di = binding.DeviceInputs(prob, host=True)
+    r = binding.Refiner.for_inputs(di, prob["params"], host_path=True)
+    out = r.run(di, prob["params"])
+    for k in ("poses", "cost", "iter_hessian"):
+        assert np.array_equal(out[k].numpy(), dev[k]), k
+    r.close()
