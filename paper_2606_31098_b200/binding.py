@@ -228,7 +228,7 @@ class Refiner:
     def for_inputs(cls, di, params, device=0, host_path=False):
         P = dict(DEFAULT_PARAMS); P.update(params or {})
         dsm = (int(di.inp.dsm_width), int(di.inp.dsm_height))
-        return cls(di.n_levels, di.width, di.height, di.channels, di.dtype, di.n_hyp, di.max_points,
+        return cls(di.n_levels, di.width, di.height, di.channels, di.dtype, max(1, di.n_hyp), max(1, di.max_points),
                    sum(P["iters"]), device=device, host_path=host_path, max_dsm=dsm)
 
     def set_chunk(self, chunk):
