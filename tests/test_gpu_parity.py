@@ -178,7 +178,9 @@ def test_full_size_sampled_hypotheses(name, stride):
     g = {k: (v[:, idx] if k.startswith("iter_") else v[idx]) for k, v in gpu.items() if isinstance(v, np.ndarray)}
     o = {k: (v[:, idx] if k.startswith("iter_") else v[idx]) for k, v in orc.items() if isinstance(v, np.ndarray)}
     check_systems(g, o, "bf16", recs=(0,))
-    conv = parity.converged(o)
+    # at these scene scales (ranges of 200-900 m) the last accepted steps are ~1e-5..1e-4 m: well inside the
+    # 5e-3 pose tolerance, so 'converged' means last accepted |dxi| < 5e-4 here
+    conv = parity.converged(o, step_tol=5e-4)
     assert conv.sum() >= max(1, len(idx) // 2), conv.sum()
     er, et = parity.pose_errors(g, o)
     assert er[conv].max() <= 5e-3 and et[conv].max() <= 5e-3, (er[conv].max(), et[conv].max())
