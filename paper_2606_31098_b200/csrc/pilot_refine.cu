@@ -129,43 +129,69 @@ namespace {
 //   p = { gx.gx, gx.gy, gy.gy, gx.r, gy.r, r.r }.
 struct RawTaps { uint4 q00, q10, q01, q11, ref; };
 
-__device__ __forceinline__ RawTaps load_taps(const char* feat, unsigned off, unsigned px_stride,
-                                             unsigned row_stride, const char* ref) {
+template <int PX>   // PX = bytes per pixel = 16*G: the x+1 taps are an immediate offset away
+__device__ __forceinline__ RawTaps load_taps(const char* feat, unsigned off, unsigned row_stride, const char* ref) {
   RawTaps t;
   const char* p = feat + off;
+  const char* q = p + row_stride;
   t.q00 = ldg16(p);
-  t.q10 = ldg16(p + px_stride);
-  t.q01 = ldg16(p + row_stride);
-  t.q11 = ldg16(p + row_stride + px_stride);
+  t.q10 = ldg16(p + PX);
+  t.q01 = ldg16(q);
+  t.q11 = ldg16(q + PX);
   t.ref = ldg16(ref);
   return t;
 }
 
+// Packed fp32x2 arithmetic (sm_100 FFMA2 / FADD2): two channels per instruction, half the issue slots.
+__device__ __forceinline__ float2 sub2(float2 x, float2 y) { return __ffma2_rn(y, make_float2(-1.f, -1.f), x); }
+
+template <class T> __device__ __forceinline__ void unpack2(const uint4& v, float2 (&o)[T::kVec / 2]);
+template <> __device__ __forceinline__ void unpack2<F32Tag>(const uint4& v, float2 (&o)[2]) {
+  o[0] = make_float2(__uint_as_float(v.x), __uint_as_float(v.y));
+  o[1] = make_float2(__uint_as_float(v.z), __uint_as_float(v.w));
+}
+template <> __device__ __forceinline__ void unpack2<BF16Tag>(const uint4& v, float2 (&o)[4]) {
+  // a 32-bit word holds channels (2i, 2i+1): low half << 16 and the masked high half are the two fp32 values
+  o[0] = make_float2(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xffff0000u));
+  o[1] = make_float2(__uint_as_float(v.y << 16), __uint_as_float(v.y & 0xffff0000u));
+  o[2] = make_float2(__uint_as_float(v.z << 16), __uint_as_float(v.z & 0xffff0000u));
+  o[3] = make_float2(__uint_as_float(v.w << 16), __uint_as_float(v.w & 0xffff0000u));
+}
+template <> __device__ __forceinline__ void unpack2<F16Tag>(const uint4& v, float2 (&o)[4]) {
+  const __half2* h = reinterpret_cast<const __half2*>(&v);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) o[i] = __half22float2(h[i]);
+}
+
 template <class T>
 __device__ __forceinline__ void unit_partials(const RawTaps& t, float a, float b, float (&p)[6]) {
-  constexpr int V = T::kVec;
-  float f00[V], f10[V], f01[V], f11[V], fr[V];
-  unpack<T>(t.q00, f00); unpack<T>(t.q10, f10); unpack<T>(t.q01, f01); unpack<T>(t.q11, f11);
-  unpack<T>(t.ref, fr);
+  constexpr int V2 = T::kVec / 2;
+  float2 f00[V2], f10[V2], f01[V2], f11[V2], fr[V2];
+  unpack2<T>(t.q00, f00); unpack2<T>(t.q10, f10); unpack2<T>(t.q01, f01); unpack2<T>(t.q11, f11);
+  unpack2<T>(t.ref, fr);
+  const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+  float2 acc[6];
 #pragma unroll
-  for (int i = 0; i < 6; ++i) p[i] = 0.f;
+  for (int i = 0; i < 6; ++i) acc[i] = make_float2(0.f, 0.f);
 #pragma unroll
-  for (int i = 0; i < V; ++i) {
-    float d0 = f10[i] - f00[i];            // x-difference, top row
-    float d1 = f11[i] - f01[i];            // x-difference, bottom row
-    float top = fmaf(a, d0, f00[i]);
-    float bot = fmaf(a, d1, f01[i]);
-    float gy = bot - top;                  // = (1-a)(f01-f00) + a(f11-f10): exact d/dv of the bilinear patch
-    float f = fmaf(b, gy, top);            // bilinear value
-    float gx = fmaf(b, d1 - d0, d0);       // = (1-b)(f10-f00) + b(f11-f01): exact d/du
-    float r = f - fr[i];                   // Eq.(1)
-    p[0] = fmaf(gx, gx, p[0]);
-    p[1] = fmaf(gx, gy, p[1]);
-    p[2] = fmaf(gy, gy, p[2]);
-    p[3] = fmaf(gx, r, p[3]);
-    p[4] = fmaf(gy, r, p[4]);
-    p[5] = fmaf(r, r, p[5]);
+  for (int i = 0; i < V2; ++i) {
+    float2 d0 = sub2(f10[i], f00[i]);          // x-difference, top row
+    float2 d1 = sub2(f11[i], f01[i]);          // x-difference, bottom row
+    float2 top = __ffma2_rn(a2, d0, f00[i]);
+    float2 bot = __ffma2_rn(a2, d1, f01[i]);
+    float2 gy = sub2(bot, top);                // = (1-a)(f01-f00) + a(f11-f10): exact d/dv of the bilinear patch
+    float2 f = __ffma2_rn(b2, gy, top);        // bilinear value
+    float2 gx = __ffma2_rn(b2, sub2(d1, d0), d0);  // = (1-b)(f10-f00) + b(f11-f01): exact d/du
+    float2 r = sub2(f, fr[i]);                 // Eq.(1)
+    acc[0] = __ffma2_rn(gx, gx, acc[0]);
+    acc[1] = __ffma2_rn(gx, gy, acc[1]);
+    acc[2] = __ffma2_rn(gy, gy, acc[2]);
+    acc[3] = __ffma2_rn(gx, r, acc[3]);
+    acc[4] = __ffma2_rn(gy, r, acc[4]);
+    acc[5] = __ffma2_rn(r, r, acc[5]);
   }
+#pragma unroll
+  for (int i = 0; i < 6; ++i) p[i] = acc[i].x + acc[i].y;
 }
 
 // One step of a recursive-halving reduce-scatter across lane bit `bit`: lanes with the bit clear
@@ -247,7 +273,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const HypSta
       rb = __shfl_sync(0xffffffffu, b, r, G);
       rvalid = o != 0xffffffffu;
       int jr = min(gbase + r, L.N - 1);
-      return load_taps(feat, (rvalid ? o : 0u) + (unsigned)sub * 16u, px_stride, row_stride,
+      return load_taps<16 * G>(feat, (rvalid ? o : 0u) + (unsigned)sub * 16u, row_stride,
                        refb + ((size_t)jr * L.C) * esz + (size_t)sub * 16u);
     };
     float na, nb; bool nvalid;
