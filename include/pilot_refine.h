@@ -168,6 +168,68 @@ int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk);
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */
 int pilot_refine_last_launches(const pilot_refine_handle* h);
 
+/*
+ * The same as pilot_refine_run restricted to pyramid levels level_begin <= l < level_end
+ * (0 <= level_begin < level_end <= n_levels): what the paper's schedule needs to prune the
+ * hypothesis set between the coarse and the finer levels (supp II-C).
+ * The final outputs (poses/cost/n_valid/status) describe the accepted state at level
+ * level_end-1. The iter_* records keep the layout of the whole run: record index =
+ * sum(iters[0..l-1]) + k for every level l (levels outside the range are left untouched),
+ * with H = in->n_hypotheses of THIS call. pilot_refine_run == run_levels(0, n_levels).
+ */
+int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* in,
+                            const pilot_refine_params* p, const pilot_refine_outputs* out,
+                            int level_begin, int level_end, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Hypothesis set: sampling, pruning, selection ("sample multiple pose hypotheses in
+ * the local (x,y,psi) space around the propagated pose prior"; supp II-C PAPER.md:381-386: +-10 m
+ * grid with 2 m step x yaw offsets {+-1,+-3,+-5,+-7,+-9} deg = 1210 hypotheses, top 128 by
+ * post-update objective kept after the coarse level; "the hypothesis with the lowest
+ * final objective value is selected"). All asynchronous on `cuda_stream`, no allocation, no sync.
+ */
+typedef enum {
+  PILOT_SEED_CAMERA = 0,  /* R_wc,m = R_wc Rot(w_m): rotation offset expressed in the camera frame */
+  PILOT_SEED_WORLD  = 1   /* R_wc,m = Rot(w_m) R_wc: rotation offset in the world frame (yaw = w || vertical) */
+} pilot_seed_frame;
+
+/*
+ * Pure host helper: fills offsets_host[n][6] = (w_x,w_y,w_z rotation vector in radians; t_x,t_y,t_z in
+ * metres) with the paper's grid: t = (i*xy_step, j*xy_step, 0) for i,j in [-r, r], r = floor(xy_range /
+ * xy_step + 1e-6), and w = radians(yaw_deg[k]) * up (PILOT_SEED_WORLD offsets; `up` = unit vertical,
+ * typically -gamma^W). Order: index = ((i+r)*(2r+1) + (j+r))*n_yaw + k. Returns the number of entries
+ * ((2r+1)^2 * n_yaw; 1210 for 10 m / 2 m / 10 yaws) — also when offsets_host is NULL or capacity is too
+ * small (nothing is written then) — or a negative PILOT_ERR_ARG.
+ */
+int pilot_refine_grid_offsets(float xy_range, float xy_step, const float* yaw_deg, int n_yaw,
+                              const float up[3], float* offsets_host, int capacity);
+
+/*
+ * out_poses_dev[m] = base pose composed with offsets_dev[m] (m < n): rotation per `frame` above,
+ * centre C_m = C + t_m. base_pose_dev: [12] row-major [R_wc | C]; offsets_dev: [n][6]; out: [n][12].
+ */
+int pilot_refine_seed_hypotheses(const float* base_pose_dev, const float* offsets_dev, int n, int frame,
+                                 float* out_poses_dev, void* cuda_stream);
+
+/*
+ * Index of the lowest cost among n (NaN counts as +inf; ties -> lowest index; n >= 1). Writes (each
+ * optional, may be NULL): best_idx_dev[1], best_pose_dev[12] (copied from poses_dev[best]),
+ * best_cost_dev[1].
+ */
+int pilot_refine_select_best(const float* cost_dev, const float* poses_dev, int n,
+                             int* best_idx_dev, float* best_pose_dev, float* best_cost_dev,
+                             void* cuda_stream);
+
+/*
+ * The k hypotheses of lowest cost, in ascending (cost, index) order (NaN = +inf): idx_out_dev[k],
+ * and optionally their poses (poses_out_dev[k][12] gathered from poses_dev) and costs
+ * (cost_out_dev[k]). 1 <= k <= n <= PILOT_TOPK_MAX, else PILOT_ERR_UNSUPPORTED.
+ */
+#define PILOT_TOPK_MAX 8192
+int pilot_refine_prune_topk(const float* cost_dev, const float* poses_dev, int n, int k,
+                            int* idx_out_dev, float* poses_out_dev, float* cost_out_dev,
+                            void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif
