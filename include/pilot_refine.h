@@ -230,6 +230,67 @@ int pilot_refine_prune_topk(const float* cost_dev, const float* poses_dev, int n
                             int* idx_out_dev, float* poses_out_dev, float* cost_out_dev,
                             void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Streaming sequence ("we use the pose estimated from the previous query image as the pose
+ * prior"; supp IV PAPER.md:457-461: the reference of the NEXT frame is prepared asynchronously while the
+ * current frame is localised). A sequence object owns: one refinement handle, the static heightfield, a
+ * DOUBLE BUFFER of per-frame device inputs filled from host memory on the library's own copy stream, the
+ * hypothesis-offset table, and an on-device log of per-frame results. Per frame, on the caller's compute
+ * stream and without any host synchronisation:
+ *     hypotheses = previous estimate (x) offsets  ->  pilot_refine_run  ->  arg-min  ->  new estimate, log row.
+ * upload() of frame i+1 may be issued before step() of frame i: the copy overlaps the refinement; events
+ * order slot reuse. upload() first copies the caller's arrays into page-locked staging owned by the object, so
+ * they may be pageable and may be reused as soon as upload() returns.
+ */
+typedef struct pilot_refine_sequence pilot_refine_sequence; /* opaque */
+
+typedef struct {
+  int n_hypotheses;                    /* H per frame, <= cfg.max_hypotheses */
+  const float* offsets;                /* HOST [H][6] (rotation vector rad, translation m), see pilot_refine_seed_hypotheses */
+  int seed_frame;                      /* pilot_seed_frame */
+  const float* dsm;                    /* HOST [dsm_height][dsm_width] heightfield, uploaded once (NULL: no range prior) */
+  int dsm_width, dsm_height;
+  float dsm_origin_x, dsm_origin_y, dsm_gsd;
+  float gravity_world[3];
+  int max_frames;                      /* capacity of the result log */
+} pilot_refine_sequence_config;
+
+typedef struct {                       /* one frame; HOST pointers, same layouts as pilot_refine_inputs */
+  int n_points[PILOT_MAX_LEVELS];
+  const void*  query_feat[PILOT_MAX_LEVELS];
+  const float* query_conf[PILOT_MAX_LEVELS];      /* NULL = 1 */
+  const float* points[PILOT_MAX_LEVELS];
+  const void*  ref_feat[PILOT_MAX_LEVELS];
+  float intrinsics[PILOT_MAX_LEVELS][4];
+  float gravity_imu[3], range_ray_cam[3], range_meas;
+} pilot_refine_frame;
+
+#define PILOT_SEQ_ROW 16               /* floats per log row: pose[12], cost, best index, n_valid, status */
+
+/* Allocates everything once (cudaMalloc, cudaHostAlloc, one copy stream, events). cfg->workspace_dev must be NULL. */
+int pilot_refine_sequence_create(const pilot_refine_config* cfg, const pilot_refine_sequence_config* sc,
+                                 pilot_refine_sequence** out);
+/* Sets the pose prior of the next frame (frame 0: e.g. the last GNSS fix). pose_host: [12]. */
+int pilot_refine_sequence_set_prior(pilot_refine_sequence* s, const float* pose_host, void* cuda_stream);
+/* Stages one frame (host memcpy) and enqueues its host->device copy into the free half of the double buffer on
+ * the copy stream. Returns PILOT_ERR_UNSUPPORTED if both halves hold frames that were not stepped yet.
+ * Asynchronous w.r.t. the device (may wait on the host for the copy issued two uploads earlier). */
+int pilot_refine_sequence_upload(pilot_refine_sequence* s, const pilot_refine_frame* f);
+/* Refines the oldest uploaded frame on `cuda_stream` (waits for its copy by event). Asynchronous.
+ * PILOT_ERR_ARG if no uploaded frame is pending or the log is full. */
+int pilot_refine_sequence_step(pilot_refine_sequence* s, const pilot_refine_params* p, void* cuda_stream);
+/* Copies log rows [first, first+count) to results_host[count][PILOT_SEQ_ROW] and synchronises `cuda_stream`. */
+int pilot_refine_sequence_results(pilot_refine_sequence* s, int first, int count, float* results_host,
+                                  void* cuda_stream);
+/* The LAST stepped frame's hypothesis set: seeds [H][12], refined poses [H][12], costs [H] (each optional) to
+ * host memory; synchronises `cuda_stream`. For inspection and parity tests. */
+int pilot_refine_sequence_last_frame(pilot_refine_sequence* s, float* seeds_host, float* poses_host,
+                                     float* cost_host, void* cuda_stream);
+/* Kernel launches enqueued by the last step(). */
+int pilot_refine_sequence_last_launches(const pilot_refine_sequence* s);
+/* Waits for both streams' pending work of this object, then frees everything. destroy(NULL) is a no-op. */
+int pilot_refine_sequence_destroy(pilot_refine_sequence* s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,8 +20,17 @@ DAMP_CODE = {"identity": 0, "diag": 1}
 GRAD_CODE = {"bilinear_exact": 0, "central_sampled": 1}
 ERRORS = {-1: "bad argument", -2: "workspace too small", -3: "unsupported shape / mode", -4: "CUDA error"}
 
+SEED_CODE = {"camera": 0, "world": 1}
+TOPK_MAX = 8192
+
 EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy",
-           "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_last_launches"]
+           "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_last_launches",
+           "pilot_refine_run_levels", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
+           "pilot_refine_select_best", "pilot_refine_prune_topk",
+           "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
+           "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
+           "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy"]
+SEQ_ROW = 16
 
 
 class Config(C.Structure):
@@ -62,6 +71,21 @@ class Outputs(C.Structure):
                 ("iter_lambda_dev", C.c_void_p)]
 
 
+class SequenceConfig(C.Structure):
+    _fields_ = [("n_hypotheses", C.c_int), ("offsets", C.c_void_p), ("seed_frame", C.c_int),
+                ("dsm", C.c_void_p), ("dsm_width", C.c_int), ("dsm_height", C.c_int),
+                ("dsm_origin_x", C.c_float), ("dsm_origin_y", C.c_float), ("dsm_gsd", C.c_float),
+                ("gravity_world", C.c_float * 3), ("max_frames", C.c_int)]
+
+
+class Frame(C.Structure):
+    _fields_ = [("n_points", C.c_int * MAX_LEVELS),
+                ("query_feat", C.c_void_p * MAX_LEVELS), ("query_conf", C.c_void_p * MAX_LEVELS),
+                ("points", C.c_void_p * MAX_LEVELS), ("ref_feat", C.c_void_p * MAX_LEVELS),
+                ("intrinsics", (C.c_float * 4) * MAX_LEVELS),
+                ("gravity_imu", C.c_float * 3), ("range_ray_cam", C.c_float * 3), ("range_meas", C.c_float)]
+
+
 DEFAULT_PARAMS = dict(
     iters=[10], loss="huber", loss_scale=0.1, lm_mode="adaptive", damp_mode="identity",
     lambda_init=1e-2, lambda_up=10.0, lambda_down=0.1, lambda_min=1e-8, lambda_max=1e8,
@@ -96,6 +120,31 @@ def lib():
         L.pilot_refine_last_launches.restype = C.c_int
         L.pilot_refine_set_chunk.argtypes = [C.c_void_p, C.c_int]
         L.pilot_refine_set_chunk.restype = C.c_int
+        L.pilot_refine_run_levels.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.POINTER(Outputs),
+                                              C.c_int, C.c_int, C.c_void_p]
+        L.pilot_refine_run_levels.restype = C.c_int
+        L.pilot_refine_grid_offsets.argtypes = [C.c_float, C.c_float, C.POINTER(C.c_float), C.c_int,
+                                                C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int]
+        L.pilot_refine_grid_offsets.restype = C.c_int
+        L.pilot_refine_seed_hypotheses.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.pilot_refine_seed_hypotheses.restype = C.c_int
+        L.pilot_refine_select_best.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_void_p]
+        L.pilot_refine_select_best.restype = C.c_int
+        L.pilot_refine_prune_topk.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                              C.c_void_p, C.c_void_p]
+        L.pilot_refine_prune_topk.restype = C.c_int
+        L.pilot_refine_sequence_create.argtypes = [C.POINTER(Config), C.POINTER(SequenceConfig), C.POINTER(C.c_void_p)]
+        L.pilot_refine_sequence_set_prior.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_sequence_upload.argtypes = [C.c_void_p, C.POINTER(Frame)]
+        L.pilot_refine_sequence_step.argtypes = [C.c_void_p, C.POINTER(Params), C.c_void_p]
+        L.pilot_refine_sequence_results.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.pilot_refine_sequence_last_frame.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_sequence_last_launches.argtypes = [C.c_void_p]
+        L.pilot_refine_sequence_destroy.argtypes = [C.c_void_p]
+        for name in EXPORTS:
+            if name.startswith("pilot_refine_sequence_"):
+                getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
 
@@ -235,8 +284,9 @@ class Refiner:
         _check(lib().pilot_refine_set_chunk(self.handle, int(chunk)), "pilot_refine_set_chunk")
 
     def run(self, di, params, stream=None, outputs=("poses", "cost", "n_valid", "status", "iter_hessian",
-                                                    "iter_gradient", "iter_cost", "iter_lambda")):
-        """Enqueue one refinement. Returns dict of output tensors (views; valid once the stream reaches them)."""
+                                                    "iter_gradient", "iter_cost", "iter_lambda"), levels=None):
+        """Enqueue one refinement (of pyramid levels [levels[0], levels[1]) if given). Returns dict of output
+        tensors (views; valid once the stream reaches them)."""
         torch = self.torch
         par, P = make_params(params, di.n_levels)
         out = Outputs()
@@ -244,9 +294,15 @@ class Refiner:
             setattr(out, name + "_dev", self.o[name].data_ptr())
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
-        fn = lib().pilot_refine_run_host if self.host_path else lib().pilot_refine_run
-        _check(fn(self.handle, C.byref(di.inp), C.byref(par), C.byref(out), C.c_void_p(stream.cuda_stream)),
-               "pilot_refine_run_host" if self.host_path else "pilot_refine_run")
+        if levels is not None:
+            assert not self.host_path, "run_levels has no host-buffer variant"
+            _check(lib().pilot_refine_run_levels(self.handle, C.byref(di.inp), C.byref(par), C.byref(out),
+                                                 int(levels[0]), int(levels[1]), C.c_void_p(stream.cuda_stream)),
+                   "pilot_refine_run_levels")
+        else:
+            fn = lib().pilot_refine_run_host if self.host_path else lib().pilot_refine_run
+            _check(fn(self.handle, C.byref(di.inp), C.byref(par), C.byref(out), C.c_void_p(stream.cuda_stream)),
+                   "pilot_refine_run_host" if self.host_path else "pilot_refine_run")
         H, T = di.n_hyp, sum(P["iters"])
         res = {}
         for name in outputs:
@@ -287,3 +343,182 @@ def refine(prob, params=None, device=0):
     res["launches"] = r.last_launches
     r.close()
     return res
+
+
+# ------------------------------------------------------------------ hypothesis set
+
+def grid_offsets(xy_range, xy_step, yaw_deg, up):
+    """The paper's (x, y, psi) grid as [n, 6] float32 (rotation vector rad, translation m); pure host call."""
+    yaw = (C.c_float * len(yaw_deg))(*[float(y) for y in yaw_deg])
+    upv = (C.c_float * 3)(*[float(v) for v in up])
+    n = lib().pilot_refine_grid_offsets(float(xy_range), float(xy_step), yaw, len(yaw_deg), upv, None, 0)
+    if n < 0:
+        _check(n, "pilot_refine_grid_offsets")
+    out = np.zeros((n, 6), np.float32)
+    n2 = lib().pilot_refine_grid_offsets(float(xy_range), float(xy_step), yaw, len(yaw_deg), upv,
+                                         out.ctypes.data_as(C.POINTER(C.c_float)), n)
+    assert n2 == n
+    return out
+
+
+def _stream_ptr(torch, stream, device):
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+    return C.c_void_p(stream.cuda_stream)
+
+
+def seed_hypotheses(base_pose, offsets, frame="camera", out=None, stream=None):
+    """base_pose: cuda float32 [12]; offsets: cuda float32 [n, 6] -> cuda float32 [n, 12] (asynchronous)."""
+    torch = _torch()
+    n = int(offsets.shape[0])
+    assert base_pose.is_cuda and offsets.is_cuda and base_pose.dtype == offsets.dtype == torch.float32
+    assert base_pose.is_contiguous() and offsets.is_contiguous()
+    if out is None:
+        out = torch.empty(n, 12, dtype=torch.float32, device=offsets.device)
+    _check(lib().pilot_refine_seed_hypotheses(base_pose.data_ptr(), offsets.data_ptr(), n, SEED_CODE[frame],
+                                              out.data_ptr(), _stream_ptr(torch, stream, offsets.device)),
+           "pilot_refine_seed_hypotheses")
+    return out
+
+
+def select_best(cost, poses, stream=None):
+    """cost: cuda float32 [n]; poses: cuda float32 [n, 12] -> (idx int32 [1], pose [12], cost [1]) on the device."""
+    torch = _torch()
+    n = int(cost.shape[0])
+    assert cost.is_cuda and cost.dtype == torch.float32 and cost.is_contiguous() and poses.is_contiguous()
+    idx = torch.empty(1, dtype=torch.int32, device=cost.device)
+    pose = torch.empty(12, dtype=torch.float32, device=cost.device)
+    bc = torch.empty(1, dtype=torch.float32, device=cost.device)
+    _check(lib().pilot_refine_select_best(cost.data_ptr(), poses.data_ptr(), n, idx.data_ptr(), pose.data_ptr(),
+                                          bc.data_ptr(), _stream_ptr(torch, stream, cost.device)),
+           "pilot_refine_select_best")
+    return idx, pose, bc
+
+
+def prune_topk(cost, poses, k, stream=None):
+    """The k lowest-cost hypotheses in ascending (cost, index) order -> (idx int32 [k], poses [k, 12], cost [k])."""
+    torch = _torch()
+    n = int(cost.shape[0])
+    assert cost.is_cuda and cost.dtype == torch.float32 and cost.is_contiguous() and poses.is_contiguous()
+    idx = torch.empty(k, dtype=torch.int32, device=cost.device)
+    po = torch.empty(k, 12, dtype=torch.float32, device=cost.device)
+    co = torch.empty(k, dtype=torch.float32, device=cost.device)
+    _check(lib().pilot_refine_prune_topk(cost.data_ptr(), poses.data_ptr(), n, int(k), idx.data_ptr(), po.data_ptr(),
+                                         co.data_ptr(), _stream_ptr(torch, stream, cost.device)),
+           "pilot_refine_prune_topk")
+    return idx, po, co
+
+
+# ------------------------------------------------------------------ streaming sequence (PAPER.md:110, 457-461)
+
+def make_frame(prob):
+    """A frame problem dict (host numpy arrays) -> (Frame struct, keep-alive list, bytes uploaded per frame)."""
+    f, keep, nbytes = Frame(), [], 0
+    L = int(prob["n_levels"])
+    for l in range(L):
+        def hold(a, dt=None):
+            a = np.ascontiguousarray(a if dt is None else np.asarray(a, dt))
+            keep.append(a)
+            return a
+        q = hold(prob["query_feat"][l])
+        f.query_feat[l] = q.ctypes.data
+        nbytes += q.nbytes
+        qc = prob.get("query_conf", [None] * L)[l]
+        if qc is not None:
+            qc = hold(qc, np.float32)
+            f.query_conf[l] = qc.ctypes.data
+            nbytes += qc.nbytes
+        pts = hold(prob["points"][l], np.float32)
+        f.n_points[l] = pts.shape[0]
+        f.points[l] = pts.ctypes.data if pts.size else None
+        rf = hold(prob["ref_feat"][l])
+        f.ref_feat[l] = rf.ctypes.data if rf.size else None
+        nbytes += pts.nbytes + rf.nbytes
+        for k in range(4):
+            f.intrinsics[l][k] = float(prob["intrinsics"][l][k])
+    for k in range(3):
+        f.gravity_imu[k] = float(prob["gravity_imu"][k])
+        f.range_ray_cam[k] = float(prob["range_ray_cam"][k])
+    f.range_meas = float(prob["range_meas"])
+    return f, keep, nbytes
+
+
+class Sequence:
+    """Owns one pilot_refine_sequence: upload(frame i+1) overlaps step(frame i); everything is asynchronous until
+    results() / last_frame() are read."""
+
+    def __init__(self, n_levels, width, height, channels, dtype, n_hypotheses, max_points, total_iters, offsets,
+                 dsm, dsm_origin, dsm_gsd, gravity_world, max_frames, seed_frame="camera", device=0):
+        torch = _torch()
+        self.torch, self.device = torch, device
+        cfg = Config()
+        cfg.device, cfg.n_levels, cfg.feat_dtype = device, n_levels, DTYPE_CODE[dtype]
+        for l in range(n_levels):
+            cfg.width[l], cfg.height[l], cfg.channels[l] = int(width[l]), int(height[l]), int(channels[l])
+        cfg.max_hypotheses, cfg.max_points, cfg.max_total_iters = int(n_hypotheses), int(max_points), int(total_iters)
+        sc = SequenceConfig()
+        off = np.ascontiguousarray(offsets, np.float32).reshape(-1, 6)
+        assert off.shape[0] == n_hypotheses
+        sc.n_hypotheses, sc.offsets, sc.seed_frame = int(n_hypotheses), off.ctypes.data, SEED_CODE[seed_frame]
+        if dsm is not None:
+            d = np.ascontiguousarray(dsm, np.float32)
+            sc.dsm, sc.dsm_height, sc.dsm_width = d.ctypes.data, d.shape[0], d.shape[1]
+        sc.dsm_origin_x, sc.dsm_origin_y, sc.dsm_gsd = float(dsm_origin[0]), float(dsm_origin[1]), float(dsm_gsd)
+        for k in range(3):
+            sc.gravity_world[k] = float(gravity_world[k])
+        sc.max_frames = int(max_frames)
+        self.n_hyp, self.n_levels, self.max_frames = int(n_hypotheses), n_levels, int(max_frames)
+        self.handle = C.c_void_p()
+        _check(lib().pilot_refine_sequence_create(C.byref(cfg), C.byref(sc), C.byref(self.handle)),
+               "pilot_refine_sequence_create")
+
+    def _stream(self, stream):
+        return _stream_ptr(self.torch, stream, self.device)
+
+    def set_prior(self, pose, stream=None):
+        p = np.ascontiguousarray(pose, np.float32).reshape(12)
+        _check(lib().pilot_refine_sequence_set_prior(self.handle, p.ctypes.data, self._stream(stream)),
+               "pilot_refine_sequence_set_prior")
+
+    def upload(self, frame_prob):
+        """Stage + enqueue the H2D copy of one frame (problem dict or a (Frame, keep, nbytes) tuple of make_frame)."""
+        f = frame_prob if isinstance(frame_prob, tuple) else make_frame(frame_prob)
+        _check(lib().pilot_refine_sequence_upload(self.handle, C.byref(f[0])), "pilot_refine_sequence_upload")
+        return f[2]
+
+    def step(self, params, stream=None):
+        par, _ = make_params(params, self.n_levels)
+        _check(lib().pilot_refine_sequence_step(self.handle, C.byref(par), self._stream(stream)),
+               "pilot_refine_sequence_step")
+
+    def results(self, first=0, count=None, stream=None):
+        """Log rows [first, first+count) as numpy [count, 16]: pose[12], cost, best index, n_valid, status. Syncs."""
+        count = self.max_frames - first if count is None else count
+        out = np.zeros((count, SEQ_ROW), np.float32)
+        _check(lib().pilot_refine_sequence_results(self.handle, int(first), int(count), out.ctypes.data,
+                                                   self._stream(stream)), "pilot_refine_sequence_results")
+        return out
+
+    def last_frame(self, stream=None):
+        """(seeds [H,12], refined poses [H,12], costs [H]) of the last stepped frame. Syncs."""
+        H = self.n_hyp
+        seeds, poses, cost = np.zeros((H, 12), np.float32), np.zeros((H, 12), np.float32), np.zeros(H, np.float32)
+        _check(lib().pilot_refine_sequence_last_frame(self.handle, seeds.ctypes.data, poses.ctypes.data,
+                                                      cost.ctypes.data, self._stream(stream)),
+               "pilot_refine_sequence_last_frame")
+        return seeds, poses, cost
+
+    @property
+    def last_launches(self):
+        return lib().pilot_refine_sequence_last_launches(self.handle)
+
+    def close(self):
+        if self.handle:
+            lib().pilot_refine_sequence_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

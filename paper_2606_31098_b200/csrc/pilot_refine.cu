@@ -61,7 +61,7 @@ struct PassArgs {
   float gw[3], gi[3], ray[3], range_meas;
   const float* dsm; int dsm_w, dsm_h; float dsm_ox, dsm_oy, dsm_gsd;
   // run
-  int n_hyp, level, n_levels, pass, iters, rec_base;
+  int n_hyp, level, level_end, pass, iters, rec_base;
   int chunk, n_chunks;
   HypState* state;
   float* partials;          // [n_hyp][n_chunks][kNacc]
@@ -617,7 +617,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, int m, const float* sums 
     s.k = 0; s.pending = 0; s.lambda = (double)P.lambda_init;
     for (int i = 0; i < 9; ++i) s.Rc[i] = s.R[i];
     for (int i = 0; i < 3; ++i) s.Cc[i] = s.C[i];
-    if (A.level + 1 == A.n_levels) write_final(A, s, m);
+    if (A.level + 1 == A.level_end) write_final(A, s, m);
   }
 }
 
@@ -674,7 +674,8 @@ __global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_const
   finalize_hypothesis(A, m, s_sum, lane);
 }
 
-__global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init) {
+__global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init,
+                                  int level_begin) {
   int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= n_hyp) return;
   HypState s;
@@ -688,7 +689,7 @@ __global__ void init_state_kernel(HypState* state, unsigned* counters, const flo
   for (int i = 0; i < 21; ++i) s.H[i] = 0.0;
   for (int i = 0; i < 6; ++i) s.g[i] = 0.0;
   s.cost = 0.0; s.lambda = lambda_init; s.n_valid = 0; s.flags = 0; s.status = 0;
-  s.level = 0; s.k = 0; s.pending = 0;
+  s.level = level_begin; s.k = 0; s.pending = 0;
   state[m] = s;
   counters[m] = 0u;
 }
@@ -851,18 +852,26 @@ int pilot_refine_last_launches(const pilot_refine_handle* h) { return h ? h->las
 
 int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
                      const pilot_refine_outputs* out, void* cuda_stream) {
+  if (!h) return PILOT_ERR_ARG;
+  return pilot_refine_run_levels(h, in, p, out, 0, h->cfg.n_levels, cuda_stream);
+}
+
+int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                            const pilot_refine_outputs* out, int level_begin, int level_end, void* cuda_stream) {
   if (!h || !in || !p || !out) return PILOT_ERR_ARG;
   const pilot_refine_config& c = h->cfg;
+  if (level_begin < 0 || level_begin >= level_end || level_end > c.n_levels) return PILOT_ERR_ARG;
   if (in->n_hypotheses < 0) return PILOT_ERR_ARG;
   if (in->n_hypotheses > c.max_hypotheses) return PILOT_ERR_UNSUPPORTED;
   int total_iters = 0;
   for (int l = 0; l < c.n_levels; ++l) {
     if (in->n_points[l] < 0 || p->iters[l] < 0) return PILOT_ERR_ARG;
+    total_iters += p->iters[l];
+    if (l < level_begin || l >= level_end) continue;       // pointers of levels outside the range are not read
     if (in->n_points[l] > c.max_points) return PILOT_ERR_UNSUPPORTED;
     if (!in->query_feat_dev[l]) return PILOT_ERR_ARG;
     if (in->n_points[l] > 0 && (!in->points_dev[l] || !in->ref_feat_dev[l])) return PILOT_ERR_ARG;
     if (((uintptr_t)in->query_feat_dev[l] | (uintptr_t)in->ref_feat_dev[l] | (uintptr_t)in->points_dev[l]) & 15) return PILOT_ERR_ARG;
-    total_iters += p->iters[l];
   }
   if (total_iters > c.max_total_iters) return PILOT_ERR_UNSUPPORTED;
   if (p->grad_mode != PILOT_GRAD_BILINEAR_EXACT) return PILOT_ERR_UNSUPPORTED;
@@ -887,17 +896,19 @@ int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in, cons
   A.range_meas = in->range_meas;
   A.dsm = in->dsm_dev; A.dsm_w = in->dsm_width; A.dsm_h = in->dsm_height;
   A.dsm_ox = in->dsm_origin_x; A.dsm_oy = in->dsm_origin_y; A.dsm_gsd = in->dsm_gsd;
-  A.n_hyp = in->n_hypotheses; A.n_levels = c.n_levels;
+  A.n_hyp = in->n_hypotheses; A.level_end = level_end;
   A.state = reinterpret_cast<HypState*>(h->ws + w.state);
   A.counters = reinterpret_cast<unsigned*>(h->ws + w.counters);
   A.partials = reinterpret_cast<float*>(h->ws + w.partials);
   A.out = *out;
 
   int launches = 0;
-  init_state_kernel<<<(A.n_hyp + 127) / 128, 128, 0, st>>>(A.state, A.counters, in->init_poses_dev, A.n_hyp, (double)p->lambda_init);
+  init_state_kernel<<<(A.n_hyp + 127) / 128, 128, 0, st>>>(A.state, A.counters, in->init_poses_dev, A.n_hyp, (double)p->lambda_init,
+                                                                  level_begin);
   ++launches;
   int rec_base = 0;
-  for (int l = 0; l < c.n_levels; ++l) {
+  for (int l = 0; l < level_end; ++l) {
+    if (l < level_begin) { rec_base += p->iters[l]; continue; }
     LevelArgs& L = A.lv;
     L.feat = in->query_feat_dev[l]; L.conf = in->query_conf_dev[l];
     L.points = reinterpret_cast<const float4*>(in->points_dev[l]); L.ref = in->ref_feat_dev[l];

@@ -24,6 +24,9 @@ The paper measured on SynthCity-6 / UAVScenes / UAVD4L-2yr with trained descript
 paper's shapes: 3-level pyramid of 32-ch descriptors, hundreds to thousands of
 anchors, 10^2-10^3 hypotheses, oblique views.
 """
+import copy
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 from scipy.ndimage import map_coordinates
 from scipy.spatial.transform import Rotation
@@ -350,6 +353,162 @@ def config4(H=256, N=65536, iters=10, width=1920, height=1080, dsm_size=4096):
     prob = _assemble("config4", rng, field, [(width, height, 64, 1.0)], "bf16", P, T_gt, K, 0.02, dsm, origin, gsd,
                      poses, params, [4])
     _sensors(prob, rng, T_gt, 0.1, 0.5, 4 * ext)
+    return prob
+
+
+# ------------------------------------------------------------------ config 3: streaming sequence
+
+def _normalize(v):
+    v = np.asarray(v, np.float64)
+    return v / np.linalg.norm(v)
+
+
+class Config3Sequence:
+    """Streaming sequence (BASELINE.json configs[3]): `n_frames` frames along a circular trajectory over one
+    2048x2048 heightfield @ 0.5 m; frames are generated lazily (`frame(i)`), each a problem dict WITHOUT init_poses
+    (the harness seeds them from the previous frame's estimate: `offsets` is the fixed table of +-5 deg / +-10 m
+    camera-frame offsets, entry 0 = identity; "pose estimated from the previous query image ... as the
+    pose prior"). Radius 300 m, 15 m/s at 30 fps, 150 m above the mean terrain, heading tangent, pitch
+    45 + 15 sin(2 pi i / 300) deg (30-60 deg oblique)."""
+
+    LEVELS = [(120, 68, 32, 0.25), (240, 135, 32, 0.5), (480, 270, 32, 1.0)]
+
+    def __init__(self, n_frames=300, H=128, N=4096, iters=(10, 10, 10), dsm_size=2048):
+        rng = _rng(3)
+        self.n_frames, self.H, self.N, self.iters = n_frames, H, N, list(iters)
+        self.gsd = 0.5
+        self.dsm = gaussian_dsm(rng, 0, dsm_size, 40 * (dsm_size // 512) ** 2, 5.0, 40.0, 8.0, 30.0, "max")
+        self.dsm64 = self.dsm.astype(np.float64)
+        self.origin = (-(dsm_size - 1) * self.gsd / 2, -(dsm_size - 1) * self.gsd / 2)
+        self.z_mean = float(self.dsm.mean())
+        self.field = SinusoidField(rng, 32, BANDS, 4)
+        self.dph = rng.uniform(-0.05, 0.05, self.field.ph.shape)           # phase drift per frame (rad)
+        self.ph0 = self.field.ph.copy()
+        f = 480 / 2 / np.tan(np.deg2rad(31.0))
+        self.K = (f, f, 240.0, 135.0)
+        off = np.zeros((H, 6), np.float32)
+        off[:, :3] = np.deg2rad(rng.uniform(-5.0, 5.0, (H, 3)))
+        off[:, 3:] = rng.uniform(-10.0, 10.0, (H, 3))
+        off[0] = 0
+        self.offsets = off
+        self.params = dict(iters=list(iters), loss="huber", loss_scale=0.1, w_gravity=1.0, gravity_scale=0.1,
+                           range_mode="march", w_range=1.0, range_scale=5.0, min_valid=max(8, N // 16))
+        self.gravity_world = np.array([0.0, 0.0, -1.0])
+        self.units_per_frame = int(sum(H * N * k for k in iters))
+
+    def gt_pose(self, i):
+        phi = 0.5 * i / 300.0                                             # 0.5 m per frame on a 300 m circle
+        C = np.array([300.0 * np.cos(phi), 300.0 * np.sin(phi), self.z_mean + 150.0])
+        pitch = 45.0 + 15.0 * np.sin(2 * np.pi * i / 300.0)
+        return pitched_pose(C, pitch, np.rad2deg(-phi))                   # heading tangent to the circle
+
+    def _height(self, x, y):
+        gx = (np.asarray(x, np.float64) - self.origin[0]) / self.gsd
+        gy = (np.asarray(y, np.float64) - self.origin[1]) / self.gsd
+        return map_coordinates(self.dsm64, [np.atleast_1d(gy), np.atleast_1d(gx)], order=1, mode="nearest")
+
+    def frame(self, i):
+        rng = np.random.Generator(np.random.PCG64([BASE_SEED + 3, i + 1]))
+        T = self.gt_pose(i)
+        # anchors: DSM nodes in a 256 m square centred on the ground point under the optical axis
+        fwd = T[:, 2]
+        t = (T[2, 3] - self.z_mean) / -fwd[2]
+        gx = (T[0, 3] + t * fwd[0] - self.origin[0]) / self.gsd
+        gy = (T[1, 3] + t * fwd[1] - self.origin[1]) / self.gsd
+        half = int(128 / self.gsd)
+        Hd, Wd = self.dsm.shape
+        region = (max(1, int(gx) - half), min(Wd - 1, int(gx) + half), max(1, int(gy) - half), min(Hd - 1, int(gy) + half))
+        P = _grid_points(rng, self.dsm, self.origin, self.gsd, self.N, region)
+        field = copy.copy(self.field)                                     # thread-safe: frames may be built in parallel
+        field.ph = self.ph0 + i * self.dph
+        prob = _assemble("config3", rng, field, self.LEVELS, "bf16", P, T, self.K, 0.02, self.dsm, self.origin,
+                         self.gsd, np.zeros((0, 12), np.float32), dict(self.params), [4, 8, 12])
+        prob.pop("init_poses")
+        prob["units"] = self.units_per_frame
+        prob["frame"] = i
+        # sensors (as _sensors, with the cached float64 heightfield)
+        e = T[:, :3].T @ self.gravity_world
+        tilt = Rotation.from_rotvec(np.deg2rad(rng.normal(0.0, 0.1, 3))).as_matrix()
+        prob["gravity_imu"] = _normalize(tilt @ e)
+        w = T[:, :3] @ prob["range_ray_cam"]
+        ts = np.linspace(0.0, 2000.0, 20001)
+        Pr = T[:, 3][None, :] + ts[:, None] * w[None, :]
+        fz = Pr[:, 2] - self._height(Pr[:, 0], Pr[:, 1])
+        k = np.nonzero((fz[:-1] > 0) & (fz[1:] <= 0))[0][0]
+        d = float(ts[k] + (ts[k + 1] - ts[k]) * fz[k] / (fz[k] - fz[k + 1]))
+        prob["range_true"] = d
+        prob["range_meas"] = float(d + rng.normal(0.0, 0.5))
+        return prob
+
+
+    def frames(self, indices=None, workers=8, ahead=16):
+        """Generator over frame dicts, built `ahead` frames in advance on a thread pool (numpy releases the GIL)."""
+        idx = list(range(self.n_frames) if indices is None else indices)
+        with ThreadPoolExecutor(max_workers=workers) as ex:
+            pending = [ex.submit(self.frame, i) for i in idx[:ahead]]
+            nxt = len(pending)
+            while pending:
+                fut = pending.pop(0)
+                if nxt < len(idx):
+                    pending.append(ex.submit(self.frame, idx[nxt]))
+                    nxt += 1
+                yield fut.result()
+
+
+def with_poses(frame_prob, poses):
+    """A frame of Config3Sequence / paper_frame plus a hypothesis set -> a complete problem dict."""
+    q = dict(frame_prob)
+    q["init_poses"] = np.ascontiguousarray(poses, np.float32).reshape(-1, 12)
+    return q
+
+
+# ------------------------------------------------------------------ paper-shaped frame (SURVEY.md §8(f).3)
+
+PAPER_YAWS = (-9.0, -7.0, -5.0, -3.0, -1.0, 1.0, 3.0, 5.0, 7.0, 9.0)      # supp Eq.(4), PAPER.md:384
+
+
+def paper_frame(N=500, iters=(2, 3, 4), dtype="bf16", prior_error=(3.1, -4.3, 2.2), range_mode="height"):
+    """The paper's own problem shape: images resized to 512, 3-level pyramid of
+    L2-normalised 32-channel descriptors with query confidence maps and per-anchor reference confidences, 500
+    geo-anchors, 2/3/4 LM iterations, 1210 (x, y, psi) hypotheses around a pose prior (to be sampled by the caller
+    from `prior_pose` with `grid = (10 m, 2 m, PAPER_YAWS)` in the world frame), top 128 kept after the coarse level.
+    Stand-in for the paper's data: analytic sinusoid descriptors, Gaussian-building DSM crop.
+    prior_error = (dx m, dy m, dyaw deg) of the prior w.r.t. the ground truth."""
+    rng = _rng(5)
+    field = SinusoidField(rng, 32, BANDS, 4)
+    dsm, origin, ext, T_gt, K = _pilot_scene(rng, 512, 0.5, 40, 512, 512)
+    P = _grid_points(rng, dsm, origin, 0.5, N)
+    params = dict(iters=list(iters), loss="huber", loss_scale=0.1, w_gravity=1.0, gravity_scale=0.1,
+                  range_mode=range_mode, w_range=1.0, range_scale=5.0, min_valid=max(8, N // 16))
+    levels = [(128, 128, 32, 0.25), (256, 256, 32, 0.5), (512, 512, 32, 1.0)]
+    prob = _assemble("paper_frame", rng, field, levels, "f32", P, T_gt, K, 0.02, dsm, origin, 0.5,
+                     np.zeros((0, 12), np.float32), params, [4, 8, 12])
+    prob.pop("init_poses")
+    # channel-wise L2 normalisation of query and reference descriptors (PAPER.md:330), then the storage dtype
+    for l in range(3):
+        q = prob["query_feat"][l].astype(np.float64)
+        prob["query_feat"][l] = encode((q / np.linalg.norm(q, axis=-1, keepdims=True)).astype(np.float32), dtype)
+        r = prob["ref_feat"][l].astype(np.float64)
+        prob["ref_feat"][l] = encode((r / np.linalg.norm(r, axis=-1, keepdims=True)).astype(np.float32), dtype)
+        W, H = prob["width"][l], prob["height"][l]
+        ys, xs = np.mgrid[0:H, 0:W] / levels[l][3]
+        conf = 1.0 / (1.0 + np.exp(-(1.0 + 1.5 * np.sin(xs / 70.0 + 0.3) * np.cos(ys / 55.0 - 0.2))))   # sigmoid head
+        prob["query_conf"][l] = conf.astype(np.float32)
+    prob["dtype"] = dtype
+    w_ref = rng.uniform(0.5, 1.0, N).astype(np.float32)
+    pts = prob["points"][0].copy()
+    pts[:, 3] = w_ref
+    prob["points"] = [pts, pts, pts]
+    _sensors(prob, rng, T_gt, 0.1, 0.5, 4 * ext)
+    dx, dy, dyaw = prior_error
+    Tp = T_gt.copy()
+    Tp[:, :3] = Rotation.from_rotvec([0.0, 0.0, np.deg2rad(dyaw)]).as_matrix() @ T_gt[:, :3]
+    Tp[:, 3] = T_gt[:, 3] + [dx, dy, 0.0]
+    prob["prior_pose"] = Tp.reshape(-1).astype(np.float32)
+    prob["grid"] = (10.0, 2.0, PAPER_YAWS)
+    prob["keep"] = 128
+    H0 = 121 * len(PAPER_YAWS)
+    prob["units"] = int(N * (H0 * iters[0] + prob["keep"] * (iters[1] + iters[2])))
     return prob
 
 
