@@ -210,7 +210,8 @@ class DeviceInputs:
             self.h2d_bytes += t.numel()
             return t.data_ptr() if t.numel() else None
 
-        self.n_hyp = int(prob["init_poses"].shape[0])
+        has_poses = prob.get("init_poses") is not None
+        self.n_hyp = int(prob["init_poses"].shape[0]) if has_poses else 0
         inp.n_hypotheses = self.n_hyp
         for l in range(L):
             inp.query_feat_dev[l] = put(prob["query_feat"][l])
@@ -222,7 +223,7 @@ class DeviceInputs:
             inp.n_points[l] = pts.shape[0]
             inp.points_dev[l] = put(pts)
             inp.ref_feat_dev[l] = put(prob["ref_feat"][l])
-        inp.init_poses_dev = put(prob["init_poses"], np.float32)
+        inp.init_poses_dev = put(prob["init_poses"], np.float32) if has_poses else None
         for k in range(3):
             inp.gravity_world[k] = float(prob["gravity_world"][k])
             inp.gravity_imu[k] = float(prob["gravity_imu"][k])
@@ -522,3 +523,53 @@ class Sequence:
             self.close()
         except Exception:
             pass
+
+
+# ------------------------------------------------------------------ the paper's multi-hypothesis schedule
+
+class PrunedRefiner:
+    """supp II-C: sample H0 hypotheses around a pose prior, refine them on the coarse level, keep
+    the `keep` lowest post-update objectives, refine those on the finer levels, return the arg-min.
+    Five C-ABI calls per frame on one stream (seed, run_levels, prune_topk, run_levels, select_best): no host sync."""
+
+    def __init__(self, di, params, offsets, keep, seed_frame="world", device=0):
+        torch = _torch()
+        self.torch, self.device, self.di, self.params = torch, device, di, dict(params)
+        off = np.ascontiguousarray(offsets, np.float32).reshape(-1, 6)
+        self.H0, self.keep, self.seed_frame = off.shape[0], int(keep), seed_frame
+        assert 1 <= self.keep <= self.H0 <= TOPK_MAX and di.n_levels >= 2
+        dev = torch.device("cuda", device)
+        self.offsets = torch.from_numpy(off).to(dev)
+        self.seeds = torch.empty(self.H0, 12, dtype=torch.float32, device=dev)
+        P = dict(DEFAULT_PARAMS); P.update(params or {})
+        self.ref = Refiner(di.n_levels, di.width, di.height, di.channels, di.dtype, self.H0, max(1, di.max_points),
+                           sum(P["iters"]), device=device)
+        self.inp0 = Inputs.from_buffer_copy(di.inp)
+        self.inp0.n_hypotheses, self.inp0.init_poses_dev = self.H0, self.seeds.data_ptr()
+        self.inp1 = Inputs.from_buffer_copy(di.inp)
+        self.inp1.n_hypotheses = self.keep
+        self.launches = 0
+
+    class _View:
+        def __init__(self, di, inp, n):
+            self.inp, self.n_hyp, self.n_levels = inp, n, di.n_levels
+
+    def run(self, prior_pose, stream=None):
+        """prior_pose: cuda float32 [12]. Returns device tensors: best_idx (into the kept set), best_pose, best_cost,
+        kept_idx [keep] (into the H0 grid), poses [keep,12], cost [keep], coarse_kept_cost [keep] (ascending)."""
+        torch, L = self.torch, self.di.n_levels
+        light = ("poses", "cost", "n_valid", "status")
+        seed_hypotheses(prior_pose, self.offsets, self.seed_frame, out=self.seeds, stream=stream)
+        o0 = self.ref.run(self._View(self.di, self.inp0, self.H0), self.params, stream, light, levels=(0, 1))
+        n = self.ref.last_launches
+        kept_idx, kept_poses, coarse_kept = prune_topk(o0["cost"], o0["poses"], self.keep, stream)
+        self.inp1.init_poses_dev = kept_poses.data_ptr()
+        o1 = self.ref.run(self._View(self.di, self.inp1, self.keep), self.params, stream, light, levels=(1, L))
+        idx, pose, bc = select_best(o1["cost"], o1["poses"], stream)
+        self.launches = n + self.ref.last_launches + 3
+        self._keepalive = kept_poses
+        return dict(best_idx=idx, best_pose=pose, best_cost=bc, kept_idx=kept_idx, poses=o1["poses"], cost=o1["cost"],
+                    n_valid=o1["n_valid"], status=o1["status"], coarse_kept_cost=coarse_kept)
+
+    def close(self):
+        self.ref.close()
