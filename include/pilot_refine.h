@@ -291,6 +291,15 @@ int pilot_refine_sequence_last_launches(const pilot_refine_sequence* s);
 /* Waits for both streams' pending work of this object, then frees everything. destroy(NULL) is a no-op. */
 int pilot_refine_sequence_destroy(pilot_refine_sequence* s);
 
+/* ---------------------------------------------------------------------------------------------
+ * Measurement helper: random-gather bandwidth of this GPU with the photo kernel's access
+ * shape — aligned reads of vec_bytes (16..512, power of two; vec_bytes/16 lanes x 16-byte ld.global.nc) at
+ * hashed positions of a buffer of buffer_bytes (e.g. 16 MiB = L2-resident, 1 GiB = HBM). Allocates and frees
+ * its own buffer, times `launches` launches with CUDA events on the default stream and SYNCHRONISES; writes
+ * the best GB/s. Not part of the refinement path.
+ */
+int pilot_refine_probe_gather(int device, size_t buffer_bytes, int vec_bytes, int launches, double* gbps_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,7 +29,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_select_best", "pilot_refine_prune_topk",
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
-           "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy"]
+           "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather"]
 SEQ_ROW = 16
 
 
@@ -142,6 +142,8 @@ def lib():
         L.pilot_refine_sequence_last_frame.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.pilot_refine_sequence_last_launches.argtypes = [C.c_void_p]
         L.pilot_refine_sequence_destroy.argtypes = [C.c_void_p]
+        L.pilot_refine_probe_gather.argtypes = [C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.pilot_refine_probe_gather.restype = C.c_int
         for name in EXPORTS:
             if name.startswith("pilot_refine_sequence_"):
                 getattr(L, name).restype = C.c_int
@@ -573,3 +575,12 @@ class PrunedRefiner:
 
     def close(self):
         self.ref.close()
+
+
+def probe_gather(buffer_bytes, vec_bytes, launches=5, device=0):
+    """Random-gather bandwidth (GB/s) of the GPU for aligned vec_bytes reads from a buffer of buffer_bytes."""
+    _torch()
+    g = C.c_double()
+    _check(lib().pilot_refine_probe_gather(int(device), int(buffer_bytes), int(vec_bytes), int(launches), C.byref(g)),
+           "pilot_refine_probe_gather")
+    return g.value

@@ -1,0 +1,85 @@
+// pilot_probe.cu — the build's own gather micro-benchmark: random, vec_bytes-aligned reads of
+// vec_bytes (one bilinear tap of C channels: 64 B for C=32 bf16, 128 B for C=64 bf16; 256/512 B for a whole
+// 2x2 footprint) from a buffer that is either L2-resident or much larger than L2. It gives the denominators the
+// photo kernel's gather is compared with: the L2->SM random-gather peak and the HBM random-gather peak (which is
+// below the streaming-copy peak of MEASURED_PEAKS.json). Same access shape as the kernel: 16-byte ld.global.nc
+// per lane, the vec_bytes/16 lanes of a group reading one contiguous vector.
+#include "../../include/pilot_refine.h"
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace {
+
+__device__ __forceinline__ uint32_t mix(uint32_t x) {          // counter-based hash (lowbias32)
+  x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+  return x;
+}
+
+template <int UNROLL>
+__global__ void __launch_bounds__(256) gather_probe_kernel(const uint4* __restrict__ buf, uint32_t n_vec, int lanes_per_vec,
+                                                           uint32_t vecs_per_thread_group, uint32_t seed, uint4* sink) {
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t group = tid / lanes_per_vec, sub = tid % lanes_per_vec;
+  uint4 acc = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = 0; i < vecs_per_thread_group; i += UNROLL) {
+    uint4 v[UNROLL];
+#pragma unroll
+    for (int u = 0; u < UNROLL; ++u) {
+      uint32_t k = mix((group * vecs_per_thread_group + i + u) ^ seed) % n_vec;
+      v[u] = __ldg(buf + (size_t)k * lanes_per_vec + sub);
+    }
+#pragma unroll
+    for (int u = 0; u < UNROLL; ++u) { acc.x ^= v[u].x; acc.y ^= v[u].y; acc.z ^= v[u].z; acc.w ^= v[u].w; }
+  }
+  if (acc.x == 0x12345678u && acc.y == 0x9abcdef0u) sink[0] = acc;   // never true in practice: keeps the loads alive
+}
+
+}  // namespace
+
+extern "C" {
+
+int pilot_refine_probe_gather(int device, size_t buffer_bytes, int vec_bytes, int launches, double* gbps_out) {
+  if (!gbps_out || launches < 1 || vec_bytes < 16 || vec_bytes > 512 || (vec_bytes & (vec_bytes - 1)) ||
+      buffer_bytes < (size_t)vec_bytes * 1024)
+    return PILOT_ERR_ARG;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (cudaSetDevice(device) != cudaSuccess) return PILOT_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaSetDevice(prev); return PILOT_ERR_CUDA; }
+  const int lanes = vec_bytes / 16;
+  const size_t n_vec = buffer_bytes / vec_bytes;
+  void *buf = nullptr, *sink = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  bool ok = n_vec <= 0xffffffffull && cudaMalloc(&buf, n_vec * vec_bytes) == cudaSuccess && cudaMalloc(&sink, 16) == cudaSuccess &&
+            cudaMemset(buf, 1, n_vec * vec_bytes) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
+            cudaEventCreate(&e1) == cudaSuccess;
+  double best = 0.0;
+  if (ok) {
+    const int ctas = prop.multiProcessorCount * 8;                 // 8 resident CTAs of 256 threads per SM
+    const uint32_t per_group = 256;                                // vectors per lane group per launch
+    const double bytes = (double)ctas * 256 / lanes * per_group * vec_bytes;
+    for (int it = 0; it < launches + 2 && ok; ++it) {              // 2 warm-up launches (also fill L2 when it fits)
+      cudaEventRecord(e0);
+      gather_probe_kernel<8><<<ctas, 256>>>(static_cast<const uint4*>(buf), (uint32_t)n_vec, lanes, per_group,
+                                           0x9e3779b9u * (uint32_t)(it + 1), static_cast<uint4*>(sink));
+      cudaEventRecord(e1);
+      ok = cudaEventSynchronize(e1) == cudaSuccess && cudaGetLastError() == cudaSuccess;
+      float ms = 0.f;
+      if (ok && it >= 2 && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess && ms > 0.f) {
+        double g = bytes / (ms * 1e-3) / 1e9;
+        if (g > best) best = g;
+      }
+    }
+  }
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  if (buf) cudaFree(buf);
+  if (sink) cudaFree(sink);
+  cudaSetDevice(prev);
+  *gbps_out = best;
+  return ok ? PILOT_OK : PILOT_ERR_CUDA;
+}
+
+}  // extern "C"
