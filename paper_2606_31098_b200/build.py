@@ -6,7 +6,8 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(CSRC, "libpilot_refine.so")
+# PILOT_REFINE_LIB: load another build of the same sources (kernel-tuning experiments); default = the in-tree library
+LIB = os.environ.get("PILOT_REFINE_LIB") or os.path.join(CSRC, "libpilot_refine.so")
 SOURCES = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 HEADERS = [os.path.join(HERE, "..", "include", "pilot_refine.h")] + sorted(glob.glob(os.path.join(CSRC, "*.cuh")))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -22,6 +23,8 @@ def _stale(target, deps):
 
 def build(force=False, verbose=False):
     """Compile every csrc/*.cu to an object (in parallel, only the stale ones) and link libpilot_refine.so."""
+    if os.environ.get("PILOT_REFINE_LIB"):
+        return LIB                      # an explicitly chosen build is used as it is
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     extra = ["-Xptxas", "-v"] if verbose else []
     objs, jobs = [], []

@@ -75,27 +75,6 @@ struct F32Tag { static constexpr int kVec = 4; };
 struct BF16Tag { static constexpr int kVec = 8; };
 struct F16Tag { static constexpr int kVec = 8; };
 
-template <class T> __device__ __forceinline__ void unpack(const uint4& v, float (&o)[T::kVec]);
-template <> __device__ __forceinline__ void unpack<F32Tag>(const uint4& v, float (&o)[4]) {
-  o[0] = __uint_as_float(v.x); o[1] = __uint_as_float(v.y);
-  o[2] = __uint_as_float(v.z); o[3] = __uint_as_float(v.w);
-}
-template <> __device__ __forceinline__ void unpack<BF16Tag>(const uint4& v, float (&o)[8]) {
-  // bf16 is the top half of an fp32: one shift / one mask per element
-  o[0] = __uint_as_float(v.x << 16); o[1] = __uint_as_float(v.x & 0xffff0000u);
-  o[2] = __uint_as_float(v.y << 16); o[3] = __uint_as_float(v.y & 0xffff0000u);
-  o[4] = __uint_as_float(v.z << 16); o[5] = __uint_as_float(v.z & 0xffff0000u);
-  o[6] = __uint_as_float(v.w << 16); o[7] = __uint_as_float(v.w & 0xffff0000u);
-}
-template <> __device__ __forceinline__ void unpack<F16Tag>(const uint4& v, float (&o)[8]) {
-  const __half2* h = reinterpret_cast<const __half2*>(&v);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    float2 f = __half22float2(h[i]);
-    o[2 * i] = f.x; o[2 * i + 1] = f.y;
-  }
-}
-
 __device__ __forceinline__ uint4 ldg16(const void* p) {
   return __ldg(reinterpret_cast<const uint4*>(p));
 }
@@ -194,6 +173,65 @@ __device__ __forceinline__ void unit_partials(const RawTaps& t, float a, float b
   for (int i = 0; i < 6; ++i) p[i] = acc[i].x + acc[i].y;
 }
 
+// GRAD_CENTRAL_SAMPLED (reading A7): gx, gy = bilinear sample (same a, b) of the central-difference
+// maps Dx[y][x] = 0.5 (F[y][min(x+1,W-1)] - F[y][max(x-1,0)]), Dy likewise (replicate border), computed on the fly
+// from the 4x4-minus-corners footprint. `nb` holds the byte offsets of the clamped outer taps relative to the
+// top-left tap: x-1 | x+2 (pixels), y-1 | y+2 (rows). The value f uses the same 2x2 taps as the default mode.
+struct OuterTaps { int xl, xr, yu, yd; };
+
+template <class T, int PX>
+__device__ __forceinline__ void unit_partials_central(const char* p00, unsigned row_stride, const OuterTaps& nb,
+                                                      const char* ref, float a, float b, float (&p)[6]) {
+  constexpr int V2 = T::kVec / 2;
+  const char* p01 = p00 + row_stride;
+  float2 f00[V2], f10[V2], f01[V2], f11[V2], t0[V2], t1[V2], t2[V2], t3[V2];
+  unpack2<T>(ldg16(p00), f00); unpack2<T>(ldg16(p00 + PX), f10);
+  unpack2<T>(ldg16(p01), f01); unpack2<T>(ldg16(p01 + PX), f11);
+  const float2 a2 = make_float2(a, a), b2 = make_float2(b, b), h2 = make_float2(0.5f, 0.5f);
+  float2 gx[V2], gy[V2], r[V2];
+  // Dx at the four taps: 0.5 (right - left); right of x0 is x0+1, left of x0+1 is x0
+  unpack2<T>(ldg16(p00 + nb.xl), t0); unpack2<T>(ldg16(p00 + nb.xr), t1);
+  unpack2<T>(ldg16(p01 + nb.xl), t2); unpack2<T>(ldg16(p01 + nb.xr), t3);
+#pragma unroll
+  for (int i = 0; i < V2; ++i) {
+    float2 dx00 = sub2(f10[i], t0[i]), dx10 = sub2(t1[i], f00[i]);
+    float2 dx01 = sub2(f11[i], t2[i]), dx11 = sub2(t3[i], f01[i]);
+    float2 top = __ffma2_rn(a2, sub2(dx10, dx00), dx00);
+    float2 bot = __ffma2_rn(a2, sub2(dx11, dx01), dx01);
+    gx[i] = __fmul2_rn(h2, __ffma2_rn(b2, sub2(bot, top), top));
+  }
+  // Dy: 0.5 (below - above); below of y0 is y0+1, above of y0+1 is y0
+  unpack2<T>(ldg16(p00 + nb.yu), t0); unpack2<T>(ldg16(p00 + nb.yd), t1);
+  unpack2<T>(ldg16(p00 + PX + nb.yu), t2); unpack2<T>(ldg16(p00 + PX + nb.yd), t3);
+#pragma unroll
+  for (int i = 0; i < V2; ++i) {
+    float2 dy00 = sub2(f01[i], t0[i]), dy01 = sub2(t1[i], f00[i]);
+    float2 dy10 = sub2(f11[i], t2[i]), dy11 = sub2(t3[i], f10[i]);
+    float2 top = __ffma2_rn(a2, sub2(dy10, dy00), dy00);
+    float2 bot = __ffma2_rn(a2, sub2(dy11, dy01), dy01);
+    gy[i] = __fmul2_rn(h2, __ffma2_rn(b2, sub2(bot, top), top));
+  }
+  unpack2<T>(ldg16(ref), t0);
+  float2 acc[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) acc[i] = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int i = 0; i < V2; ++i) {
+    float2 top = __ffma2_rn(a2, sub2(f10[i], f00[i]), f00[i]);
+    float2 bot = __ffma2_rn(a2, sub2(f11[i], f01[i]), f01[i]);
+    float2 f = __ffma2_rn(b2, sub2(bot, top), top);
+    r[i] = sub2(f, t0[i]);
+    acc[0] = __ffma2_rn(gx[i], gx[i], acc[0]);
+    acc[1] = __ffma2_rn(gx[i], gy[i], acc[1]);
+    acc[2] = __ffma2_rn(gy[i], gy[i], acc[2]);
+    acc[3] = __ffma2_rn(gx[i], r[i], acc[3]);
+    acc[4] = __ffma2_rn(gy[i], r[i], acc[4]);
+    acc[5] = __ffma2_rn(r[i], r[i], acc[5]);
+  }
+#pragma unroll
+  for (int i = 0; i < 6; ++i) p[i] = acc[i].x + acc[i].y;
+}
+
 // One step of a recursive-halving reduce-scatter across lane bit `bit`: lanes with the bit clear
 // keep `lo`, lanes with it set keep `hi`; each receives the partner's copy of what it keeps.
 template <int N>
@@ -214,10 +252,10 @@ template <> struct Log2<1> { static constexpr int v = 0; };
 // grid = (n_hyp, n_chunks): blockIdx.x (fastest) is the hypothesis, so CTAs that run together
 // sweep the SAME chunk of (spatially sorted) anchors under different poses and the union of their
 // footprints is a narrow band of the map that stays in L2.
-template <class T, int G>
+template <class T, int G, bool CEN>
 __global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_constant__ PassArgs A);
 
-template <class T, int G>
+template <class T, int G, bool CEN>
 __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const HypState* st, int chunk_idx,
                                                  float (&acc)[kNacc]) {
   constexpr int LOG = Log2<G>::v;
@@ -277,13 +315,31 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const HypSta
                        refb + ((size_t)jr * L.C) * esz + (size_t)sub * 16u);
     };
     float na, nb; bool nvalid;
-    RawTaps nxt = fetch(0, na, nb, nvalid);
+    RawTaps nxt;
+    unsigned cflags = 0;                                   // CEN: which outer taps are clamped at the border
+    if constexpr (CEN) cflags = (x0 > 0 ? 1u : 0u) | (x0 + 2 <= L.W - 1 ? 2u : 0u) | (y0 > 0 ? 4u : 0u) | (y0 + 2 <= L.H - 1 ? 8u : 0u);
+    else nxt = fetch(0, na, nb, nvalid);
 #pragma unroll
     for (int r = 0; r < G; ++r) {
-      RawTaps t = nxt;
-      float ra = na, rb = nb; bool rvalid = nvalid;
-      if (r + 1 < G) nxt = fetch(r + 1, na, nb, nvalid);   // software pipeline: next unit's loads in flight
-      unit_partials<T>(t, ra, rb, cur);
+      bool rvalid;
+      if constexpr (CEN) {
+        unsigned o = __shfl_sync(0xffffffffu, offv, r, G);
+        float ra = __shfl_sync(0xffffffffu, a, r, G), rb = __shfl_sync(0xffffffffu, b, r, G);
+        unsigned fl = __shfl_sync(0xffffffffu, cflags, r, G);
+        rvalid = o != 0xffffffffu;
+        if (!rvalid) fl = 0;                               // invisible units read around pixel (0,0), unclamped side only
+        OuterTaps ot{(fl & 1u) ? -(int)(16 * G) : 0, (fl & 2u) ? 2 * 16 * G : 16 * G,
+                     (fl & 4u) ? -(int)row_stride : 0, (fl & 8u) ? 2 * (int)row_stride : (int)row_stride};
+        int jr = min(gbase + r, L.N - 1);
+        unit_partials_central<T, 16 * G>(feat + (rvalid ? o : 0u) + (unsigned)sub * 16u, row_stride, ot,
+                                         refb + ((size_t)jr * L.C) * esz + (size_t)sub * 16u, ra, rb, cur);
+      } else {
+        RawTaps t = nxt;
+        float ra = na, rb = nb;
+        rvalid = nvalid;
+        if (r + 1 < G) nxt = fetch(r + 1, na, nb, nvalid);   // software pipeline: next unit's loads in flight
+        unit_partials<T>(t, ra, rb, cur);
+      }
       if (!rvalid) {
 #pragma unroll
         for (int i = 0; i < 6; ++i) cur[i] = 0.f;
@@ -623,7 +679,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, int m, const float* sums 
 
 // ------------------------------------------------------------------ kernels
 
-template <class T, int G>
+template <class T, int G, bool CEN>
 __global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_constant__ PassArgs A) {
   const int m = blockIdx.x, chunk_idx = blockIdx.y;
   const HypState* st = A.state + m;
@@ -632,7 +688,7 @@ __global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_const
   float acc[kNacc];
 #pragma unroll
   for (int i = 0; i < kNacc; ++i) acc[i] = 0.f;
-  photo_accumulate<T, G>(A, st, chunk_idx, acc);
+  photo_accumulate<T, G, CEN>(A, st, chunk_idx, acc);
 
   // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -752,26 +808,31 @@ WsLayout ws_layout(const pilot_refine_config* c) {
 
 typedef void (*pass_fn)(const PassArgs);
 
-template <class T>
+template <class T, bool CEN>
 pass_fn pick_g(int g) {
   switch (g) {
-    case 1: return photo_pass_kernel<T, 1>;
-    case 2: return photo_pass_kernel<T, 2>;
-    case 4: return photo_pass_kernel<T, 4>;
-    case 8: return photo_pass_kernel<T, 8>;
-    case 16: return photo_pass_kernel<T, 16>;
-    case 32: return photo_pass_kernel<T, 32>;
+    case 1: return photo_pass_kernel<T, 1, CEN>;
+    case 2: return photo_pass_kernel<T, 2, CEN>;
+    case 4: return photo_pass_kernel<T, 4, CEN>;
+    case 8: return photo_pass_kernel<T, 8, CEN>;
+    case 16: return photo_pass_kernel<T, 16, CEN>;
+    case 32: return photo_pass_kernel<T, 32, CEN>;
   }
   return nullptr;
 }
 
-pass_fn pick_kernel(pilot_dtype d, int g) {
+template <bool CEN>
+pass_fn pick_t(pilot_dtype d, int g) {
   switch (d) {
-    case PILOT_F32: return pick_g<F32Tag>(g);
-    case PILOT_BF16: return pick_g<BF16Tag>(g);
-    case PILOT_F16: return pick_g<F16Tag>(g);
+    case PILOT_F32: return pick_g<F32Tag, CEN>(g);
+    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
+    case PILOT_F16: return pick_g<F16Tag, CEN>(g);
   }
   return nullptr;
+}
+
+pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode) {
+  return grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(d, g) : pick_t<false>(d, g);
 }
 
 int choose_chunk(const pilot_refine_handle* h, int n_hyp, int n_points) {
@@ -874,7 +935,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     if (((uintptr_t)in->query_feat_dev[l] | (uintptr_t)in->ref_feat_dev[l] | (uintptr_t)in->points_dev[l]) & 15) return PILOT_ERR_ARG;
   }
   if (total_iters > c.max_total_iters) return PILOT_ERR_UNSUPPORTED;
-  if (p->grad_mode != PILOT_GRAD_BILINEAR_EXACT) return PILOT_ERR_UNSUPPORTED;
+  if (p->grad_mode != PILOT_GRAD_BILINEAR_EXACT && p->grad_mode != PILOT_GRAD_CENTRAL_SAMPLED) return PILOT_ERR_ARG;
   if (p->loss < PILOT_LOSS_L2 || p->loss > PILOT_LOSS_CAUCHY) return PILOT_ERR_ARG;
   if (p->range_mode < PILOT_RANGE_OFF || p->range_mode > PILOT_RANGE_MARCH) return PILOT_ERR_ARG;
   if (p->range_mode == PILOT_RANGE_MARCH && (p->march_steps < 1 || p->bisect_steps < 0)) return PILOT_ERR_ARG;
@@ -918,7 +979,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     A.chunk = choose_chunk(h, A.n_hyp, L.N);
     A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
     if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
-    pass_fn fn = pick_kernel(c.feat_dtype, lanes_per_unit(L.C, c.feat_dtype));
+    pass_fn fn = pick_kernel(c.feat_dtype, lanes_per_unit(L.C, c.feat_dtype), p->grad_mode);
     dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
     for (int pass = 0; pass <= p->iters[l]; ++pass) {
       A.pass = pass;

@@ -191,3 +191,42 @@ def test_full_size_sampled_hypotheses(name, stride):
     fin = np.isfinite(gpu["cost"])
     assert fin.sum() >= len(fin) // 2
     assert np.all(gpu["cost"][fin] <= gpu["iter_cost"][0][fin] * (1 + 1e-6))
+
+
+@pytest.mark.parametrize("dtype,C", [("f32", 4), ("f32", 16), ("bf16", 32), ("bf16", 64), ("f16", 8), ("bf16", 256)])
+def test_grad_central_sampled(dtype, C):
+    """Reading A7's second mode: bilinear sample of central-difference gradient maps (replicate border), on the
+    4x4-minus-corners footprint; includes units in the border cells where the outer taps are clamped."""
+    from oracle import pilot_oracle as po
+    prob = tiny(seed=40, N=1500, C=C, n_hyp=3, dtype=dtype, conf=True, W=64, H=48)
+    K = prob["intrinsics"][0]
+    prob["intrinsics"] = [(150.0, 160.0, K[2], K[3])]          # spread the anchors over (and beyond) the whole image
+    P = dict(iters=[3], loss="huber", loss_scale=0.5, grad_mode="central_sampled", min_valid=4, w_gravity=0.3)
+    # the case does exercise the clamped taps
+    b = po.Bound(prob, P)
+    R, Cc = po.pose_to_RC(prob["init_poses"][0])
+    cells = set()
+    for j in range(1500):
+        pt = po.photo_point(b, 0, R, Cc, j)
+        if pt is not None:
+            cells.add((int(np.floor(pt["uv"][0])) in (0, 62), int(np.floor(pt["uv"][1])) in (0, 46)))
+    assert (True, False) in cells and (False, True) in cells and (False, False) in cells
+    gpu, orc = both(prob, P)
+    check_systems(gpu, orc, dtype, recs=(0, 1))
+    assert np.array_equal(gpu["n_valid"], orc["n_valid"])
+    # and it is a different linearisation from the default mode
+    gpu0, _ = both(prob, dict(P, grad_mode="bilinear_exact"))
+    assert np.abs(gpu0["iter_hessian"][0] - gpu["iter_hessian"][0]).max() > 1e-3 * np.abs(gpu["iter_hessian"][0]).max()
+
+
+def test_grad_central_sampled_config0():
+    """Free-running config 0 in the central-difference mode. Here J is only approximately the derivative of the
+    sampled cost, so the accept/reject test dithers near convergence and the two trajectories
+    may take different branches: compare the first systems strictly, the end state loosely."""
+    prob = wl.config0()
+    gpu, orc = both(prob, dict(grad_mode="central_sampled", iters=[8]))
+    check_systems(gpu, orc, "f32", recs=(0, 1))
+    er, et = parity.pose_errors(gpu, orc)
+    assert er.max() <= 1e-3 and et.max() <= 2e-2
+    assert abs(gpu["cost"][0] - orc["cost"][0]) <= 1e-3 * orc["cost"][0]
+    assert gpu["cost"][0] < 0.5 * gpu["iter_cost"][0][0]
