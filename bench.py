@@ -102,6 +102,7 @@ class Resident:
         self.ref = binding.Refiner.for_inputs(self.di, self.params, local_rank)
         if args.chunk:
             self.ref.set_chunk(args.chunk)
+        self.ref.set_exec_mode(args.mode, args.cluster)
         self.H = prob["init_poses"].shape[0]
         self.units = prob["units"]
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(prob, [self.H] * prob["n_levels"])
@@ -137,6 +138,7 @@ class Resident:
         href = binding.Refiner.for_inputs(hi, self.params, self.dev, host_path=True)
         if self.args.chunk:
             href.set_chunk(self.args.chunk)
+        href.set_exec_mode(self.args.mode, self.args.cluster)
         T = sum(self.params["iters"])
         d2h = self.H * (48 + 4 + 4 + 4) + T * self.H * (144 + 24 + 4 + 4)
         href.run(hi, self.params, stream, LIGHT)
@@ -178,6 +180,7 @@ class Streaming:
             di.inp.n_hypotheses, di.n_hyp = seq.H, seq.H
             di.inp.init_poses_dev = self.seeds.data_ptr()
         self.ref = binding.Refiner.for_inputs(self.di[0], self.params, local_rank)
+        self.ref.set_exec_mode(args.mode, args.cluster)
         self.H, self.units, self.i = seq.H, seq.units_per_frame, 0
         self.prob = dict(self.frames[0], params=self.params)
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(self.prob, [self.H] * 3)
@@ -251,6 +254,7 @@ class PaperSchedule:
         self.off = binding.grid_offsets(prob["grid"][0], prob["grid"][1], prob["grid"][2], -prob["gravity_world"])
         self.di = binding.DeviceInputs(prob, local_rank)
         self.pr = binding.PrunedRefiner(self.di, self.params, self.off, prob["keep"], "world", local_rank)
+        self.pr.ref.set_exec_mode(args.mode, args.cluster)
         self.prior = torch.from_numpy(prob["prior_pose"]).to(torch.device("cuda", local_rank))
         self.H0, self.keep, self.units = self.off.shape[0], prob["keep"], prob["units"]
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(prob, [self.H0, self.keep, self.keep])
@@ -395,7 +399,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="config4", choices=sorted(WORKLOADS))
-    ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA (0 = heuristic)")
+    ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA of the pass kernel (0 = heuristic)")
+    ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident"], help="launch strategy (pilot_exec_mode)")
+    ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the gather-peak micro-benchmark")
@@ -497,7 +503,7 @@ def main():
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     if rank == 0:
-        cfg = {"workload": args.config}
+        cfg = {"workload": args.config, "exec_mode": args.mode}
         cfg.update(W.config())
         cfg.update({"map_bytes": map_bytes, "l2_bytes": int(l2_bytes),
                     "l2_policy": "L2 flushed between timed steps" if need_flush else "inputs larger than L2",

@@ -165,6 +165,16 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in_
  */
 int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk);
 
+/*
+ * Launch strategy. PASSES: one launch per EVAL pass, (hypothesis x anchor-chunk) CTAs — the throughput path for
+ * large hypothesis x anchor products. RESIDENT: one launch per pyramid level, a thread-block cluster of `cluster`
+ * CTAs (1, 2, 4, 8; 0 = heuristic) owns a hypothesis for all of the level's LM iterations — the latency path for
+ * small problems (the paper's own frame shape). AUTO (default) picks per level by H x N. Both compute the same
+ * sums from the same per-unit arithmetic; they differ in fp32 summation order only.
+ */
+typedef enum { PILOT_EXEC_AUTO = 0, PILOT_EXEC_PASSES = 1, PILOT_EXEC_RESIDENT = 2 } pilot_exec_mode;
+int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster);
+
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */
 int pilot_refine_last_launches(const pilot_refine_handle* h);
 

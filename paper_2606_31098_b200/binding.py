@@ -21,11 +21,12 @@ GRAD_CODE = {"bilinear_exact": 0, "central_sampled": 1}
 ERRORS = {-1: "bad argument", -2: "workspace too small", -3: "unsupported shape / mode", -4: "CUDA error"}
 
 SEED_CODE = {"camera": 0, "world": 1}
+EXEC_CODE = {"auto": 0, "passes": 1, "resident": 2}
 TOPK_MAX = 8192
 
 EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy",
            "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_last_launches",
-           "pilot_refine_run_levels", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
+           "pilot_refine_run_levels", "pilot_refine_set_exec_mode", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
            "pilot_refine_select_best", "pilot_refine_prune_topk",
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
@@ -120,6 +121,8 @@ def lib():
         L.pilot_refine_last_launches.restype = C.c_int
         L.pilot_refine_set_chunk.argtypes = [C.c_void_p, C.c_int]
         L.pilot_refine_set_chunk.restype = C.c_int
+        L.pilot_refine_set_exec_mode.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.pilot_refine_set_exec_mode.restype = C.c_int
         L.pilot_refine_run_levels.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.POINTER(Outputs),
                                               C.c_int, C.c_int, C.c_void_p]
         L.pilot_refine_run_levels.restype = C.c_int
@@ -283,6 +286,9 @@ class Refiner:
         return cls(di.n_levels, di.width, di.height, di.channels, di.dtype, max(1, di.n_hyp), max(1, di.max_points),
                    sum(P["iters"]), device=device, host_path=host_path, max_dsm=dsm)
 
+    def set_exec_mode(self, mode="auto", cluster=0):
+        _check(lib().pilot_refine_set_exec_mode(self.handle, EXEC_CODE[mode], int(cluster)), "pilot_refine_set_exec_mode")
+
     def set_chunk(self, chunk):
         _check(lib().pilot_refine_set_chunk(self.handle, int(chunk)), "pilot_refine_set_chunk")
 
@@ -333,12 +339,13 @@ class Refiner:
             pass
 
 
-def refine(prob, params=None, device=0):
+def refine(prob, params=None, device=0, mode="auto", cluster=0):
     """One-shot convenience: upload a problem dict, run, synchronise, return numpy outputs."""
     torch = _torch()
     di = DeviceInputs(prob, device)
     P = dict(prob.get("params", {})); P.update(params or {})
     r = Refiner.for_inputs(di, P, device)
+    r.set_exec_mode(mode, cluster)
     out = r.run(di, P)
     torch.cuda.synchronize(device)
     res = {k: v.cpu().numpy() for k, v in out.items()}

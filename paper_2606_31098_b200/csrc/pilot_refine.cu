@@ -10,685 +10,28 @@
 // candidate pose for the next pass — no host synchronisation anywhere.
 //
 // Shares no code with oracle/ (only the POD structs of include/pilot_refine.h).
-#include "../../include/pilot_refine.h"
+#include "pilot_device.cuh"
 
-#include <cuda_bf16.h>
-#include <cuda_fp16.h>
-#include <cuda_runtime.h>
-#include <math.h>
-#include <stdint.h>
 #include <stdio.h>
 #include <string.h>
 
 namespace {
 
-constexpr int kThreads = 256;            // threads per CTA of the photo kernel
-constexpr int kWarps = kThreads / 32;
-constexpr int kNacc = 32;                // 21 H + 6 g + cost + n_valid, padded to 32 floats
-constexpr int kMinChunk = kWarps * 32;   // one 32-unit batch per warp
-
-// index of the upper-triangular entry (a<=b) in the packed 21-vector
-__host__ __device__ constexpr int tri(int a, int b) { return a * 6 - a * (a - 1) / 2 + (b - a); }
-
-// Per-hypothesis optimiser state, device resident (workspace).
-struct HypState {
-  double R[9], C[3];        // accepted pose: R_cw row-major, camera centre
-  double Rc[9], Cc[3];      // candidate pose evaluated by the next pass
-  double H[21], g[6];       // accepted total system (upper triangle), undamped
-  double cost;              // accepted total cost (Eq.7)
-  double lambda;
-  int n_valid;
-  unsigned flags;           // FEW_VALID / RANGE_SKIP of the accepted state
-  unsigned status;          // sticky bits
-  int level;                // pyramid level this hypothesis is in (n_levels = finished)
-  int k;                    // solves consumed at this level
-  int pending;              // 1 if (Rc, Cc) came from a solve (not the level's first evaluation)
-};
-
-struct LevelArgs {
-  const void* feat;         // [H][W][C]
-  const float* conf;        // [H][W] or null
-  const float4* points;     // [N] xyz + w_ref
-  const void* ref;          // [N][C]
-  float fx, fy, cx, cy;
-  int W, H, C, N;
-};
-
-struct PassArgs {
-  LevelArgs lv;
-  pilot_refine_params prm;
-  // priors
-  float gw[3], gi[3], ray[3], range_meas;
-  const float* dsm; int dsm_w, dsm_h; float dsm_ox, dsm_oy, dsm_gsd;
-  // run
-  int n_hyp, level, level_end, pass, iters, rec_base;
-  int chunk, n_chunks;
-  HypState* state;
-  float* partials;          // [n_hyp][n_chunks][kNacc]
-  unsigned* counters;       // [n_hyp]
-  pilot_refine_outputs out;
-};
-
-// ------------------------------------------------------------------ element decoding
-
-struct F32Tag { static constexpr int kVec = 4; };
-struct BF16Tag { static constexpr int kVec = 8; };
-struct F16Tag { static constexpr int kVec = 8; };
-
-__device__ __forceinline__ uint4 ldg16(const void* p) {
-  return __ldg(reinterpret_cast<const uint4*>(p));
-}
-
-// ------------------------------------------------------------------ robust loss (Eq.2 / Eq.7)
-
-template <typename T>
-__device__ __forceinline__ void robust(int loss, T x, T scale, T& rho, T& drho) {
-  rho = x; drho = T(1);
-  if (scale > T(0)) {
-    T s2 = scale * scale;
-    if (loss == PILOT_LOSS_HUBER) {
-      if (x > s2) { T sq = sqrt(x); rho = T(2) * scale * sq - s2; drho = scale / sq; }
-    } else if (loss == PILOT_LOSS_CAUCHY) {
-      T q = x / s2;
-      rho = s2 * log1p(q);
-      drho = T(1) / (T(1) + q);
-    }
-  }
-}
-
-}  // namespace
-
-namespace {
-
-// ------------------------------------------------------------------ gather of one unit by a lane group
-//
-// The G = C*sizeof/16 lanes of a group own one (anchor, hypothesis) unit: each lane loads 16 B of
-// every bilinear tap (the four taps of a unit are 2 x 2 pixels x C channels = 4*C*s bytes, the
-// algorithmic gather traffic) and of the reference feature, and returns its share of
-//   p = { gx.gx, gx.gy, gy.gy, gx.r, gy.r, r.r }.
-struct RawTaps { uint4 q00, q10, q01, q11, ref; };
-
-template <int PX>   // PX = bytes per pixel = 16*G: the x+1 taps are an immediate offset away
-__device__ __forceinline__ RawTaps load_taps(const char* feat, unsigned off, unsigned row_stride, const char* ref) {
-  RawTaps t;
-  const char* p = feat + off;
-  const char* q = p + row_stride;
-  t.q00 = ldg16(p);
-  t.q10 = ldg16(p + PX);
-  t.q01 = ldg16(q);
-  t.q11 = ldg16(q + PX);
-  t.ref = ldg16(ref);
-  return t;
-}
-
-// Packed fp32x2 arithmetic (sm_100 FFMA2 / FADD2): two channels per instruction, half the issue slots.
-__device__ __forceinline__ float2 sub2(float2 x, float2 y) { return __ffma2_rn(y, make_float2(-1.f, -1.f), x); }
-
-template <class T> __device__ __forceinline__ void unpack2(const uint4& v, float2 (&o)[T::kVec / 2]);
-template <> __device__ __forceinline__ void unpack2<F32Tag>(const uint4& v, float2 (&o)[2]) {
-  o[0] = make_float2(__uint_as_float(v.x), __uint_as_float(v.y));
-  o[1] = make_float2(__uint_as_float(v.z), __uint_as_float(v.w));
-}
-template <> __device__ __forceinline__ void unpack2<BF16Tag>(const uint4& v, float2 (&o)[4]) {
-  // a 32-bit word holds channels (2i, 2i+1): low half << 16 and the masked high half are the two fp32 values
-  o[0] = make_float2(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xffff0000u));
-  o[1] = make_float2(__uint_as_float(v.y << 16), __uint_as_float(v.y & 0xffff0000u));
-  o[2] = make_float2(__uint_as_float(v.z << 16), __uint_as_float(v.z & 0xffff0000u));
-  o[3] = make_float2(__uint_as_float(v.w << 16), __uint_as_float(v.w & 0xffff0000u));
-}
-template <> __device__ __forceinline__ void unpack2<F16Tag>(const uint4& v, float2 (&o)[4]) {
-  const __half2* h = reinterpret_cast<const __half2*>(&v);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) o[i] = __half22float2(h[i]);
-}
-
-template <class T>
-__device__ __forceinline__ void unit_partials(const RawTaps& t, float a, float b, float (&p)[6]) {
-  constexpr int V2 = T::kVec / 2;
-  float2 f00[V2], f10[V2], f01[V2], f11[V2], fr[V2];
-  unpack2<T>(t.q00, f00); unpack2<T>(t.q10, f10); unpack2<T>(t.q01, f01); unpack2<T>(t.q11, f11);
-  unpack2<T>(t.ref, fr);
-  const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
-  float2 acc[6];
-#pragma unroll
-  for (int i = 0; i < 6; ++i) acc[i] = make_float2(0.f, 0.f);
-#pragma unroll
-  for (int i = 0; i < V2; ++i) {
-    float2 d0 = sub2(f10[i], f00[i]);          // x-difference, top row
-    float2 d1 = sub2(f11[i], f01[i]);          // x-difference, bottom row
-    float2 top = __ffma2_rn(a2, d0, f00[i]);
-    float2 bot = __ffma2_rn(a2, d1, f01[i]);
-    float2 gy = sub2(bot, top);                // = (1-a)(f01-f00) + a(f11-f10): exact d/dv of the bilinear patch
-    float2 f = __ffma2_rn(b2, gy, top);        // bilinear value
-    float2 gx = __ffma2_rn(b2, sub2(d1, d0), d0);  // = (1-b)(f10-f00) + b(f11-f01): exact d/du
-    float2 r = sub2(f, fr[i]);                 // Eq.(1)
-    acc[0] = __ffma2_rn(gx, gx, acc[0]);
-    acc[1] = __ffma2_rn(gx, gy, acc[1]);
-    acc[2] = __ffma2_rn(gy, gy, acc[2]);
-    acc[3] = __ffma2_rn(gx, r, acc[3]);
-    acc[4] = __ffma2_rn(gy, r, acc[4]);
-    acc[5] = __ffma2_rn(r, r, acc[5]);
-  }
-#pragma unroll
-  for (int i = 0; i < 6; ++i) p[i] = acc[i].x + acc[i].y;
-}
-
-// GRAD_CENTRAL_SAMPLED (reading A7): gx, gy = bilinear sample (same a, b) of the central-difference
-// maps Dx[y][x] = 0.5 (F[y][min(x+1,W-1)] - F[y][max(x-1,0)]), Dy likewise (replicate border), computed on the fly
-// from the 4x4-minus-corners footprint. `nb` holds the byte offsets of the clamped outer taps relative to the
-// top-left tap: x-1 | x+2 (pixels), y-1 | y+2 (rows). The value f uses the same 2x2 taps as the default mode.
-struct OuterTaps { int xl, xr, yu, yd; };
-
-template <class T, int PX>
-__device__ __forceinline__ void unit_partials_central(const char* p00, unsigned row_stride, const OuterTaps& nb,
-                                                      const char* ref, float a, float b, float (&p)[6]) {
-  constexpr int V2 = T::kVec / 2;
-  const char* p01 = p00 + row_stride;
-  float2 f00[V2], f10[V2], f01[V2], f11[V2], t0[V2], t1[V2], t2[V2], t3[V2];
-  unpack2<T>(ldg16(p00), f00); unpack2<T>(ldg16(p00 + PX), f10);
-  unpack2<T>(ldg16(p01), f01); unpack2<T>(ldg16(p01 + PX), f11);
-  const float2 a2 = make_float2(a, a), b2 = make_float2(b, b), h2 = make_float2(0.5f, 0.5f);
-  float2 gx[V2], gy[V2], r[V2];
-  // Dx at the four taps: 0.5 (right - left); right of x0 is x0+1, left of x0+1 is x0
-  unpack2<T>(ldg16(p00 + nb.xl), t0); unpack2<T>(ldg16(p00 + nb.xr), t1);
-  unpack2<T>(ldg16(p01 + nb.xl), t2); unpack2<T>(ldg16(p01 + nb.xr), t3);
-#pragma unroll
-  for (int i = 0; i < V2; ++i) {
-    float2 dx00 = sub2(f10[i], t0[i]), dx10 = sub2(t1[i], f00[i]);
-    float2 dx01 = sub2(f11[i], t2[i]), dx11 = sub2(t3[i], f01[i]);
-    float2 top = __ffma2_rn(a2, sub2(dx10, dx00), dx00);
-    float2 bot = __ffma2_rn(a2, sub2(dx11, dx01), dx01);
-    gx[i] = __fmul2_rn(h2, __ffma2_rn(b2, sub2(bot, top), top));
-  }
-  // Dy: 0.5 (below - above); below of y0 is y0+1, above of y0+1 is y0
-  unpack2<T>(ldg16(p00 + nb.yu), t0); unpack2<T>(ldg16(p00 + nb.yd), t1);
-  unpack2<T>(ldg16(p00 + PX + nb.yu), t2); unpack2<T>(ldg16(p00 + PX + nb.yd), t3);
-#pragma unroll
-  for (int i = 0; i < V2; ++i) {
-    float2 dy00 = sub2(f01[i], t0[i]), dy01 = sub2(t1[i], f00[i]);
-    float2 dy10 = sub2(f11[i], t2[i]), dy11 = sub2(t3[i], f10[i]);
-    float2 top = __ffma2_rn(a2, sub2(dy10, dy00), dy00);
-    float2 bot = __ffma2_rn(a2, sub2(dy11, dy01), dy01);
-    gy[i] = __fmul2_rn(h2, __ffma2_rn(b2, sub2(bot, top), top));
-  }
-  unpack2<T>(ldg16(ref), t0);
-  float2 acc[6];
-#pragma unroll
-  for (int i = 0; i < 6; ++i) acc[i] = make_float2(0.f, 0.f);
-#pragma unroll
-  for (int i = 0; i < V2; ++i) {
-    float2 top = __ffma2_rn(a2, sub2(f10[i], f00[i]), f00[i]);
-    float2 bot = __ffma2_rn(a2, sub2(f11[i], f01[i]), f01[i]);
-    float2 f = __ffma2_rn(b2, sub2(bot, top), top);
-    r[i] = sub2(f, t0[i]);
-    acc[0] = __ffma2_rn(gx[i], gx[i], acc[0]);
-    acc[1] = __ffma2_rn(gx[i], gy[i], acc[1]);
-    acc[2] = __ffma2_rn(gy[i], gy[i], acc[2]);
-    acc[3] = __ffma2_rn(gx[i], r[i], acc[3]);
-    acc[4] = __ffma2_rn(gy[i], r[i], acc[4]);
-    acc[5] = __ffma2_rn(r[i], r[i], acc[5]);
-  }
-#pragma unroll
-  for (int i = 0; i < 6; ++i) p[i] = acc[i].x + acc[i].y;
-}
-
-// One step of a recursive-halving reduce-scatter across lane bit `bit`: lanes with the bit clear
-// keep `lo`, lanes with it set keep `hi`; each receives the partner's copy of what it keeps.
-template <int N>
-__device__ __forceinline__ void halve(float (&lo)[N], const float (&hi)[N], int bit, bool upper) {
-#pragma unroll
-  for (int i = 0; i < N; ++i) {
-    float send = upper ? lo[i] : hi[i];
-    float keep = upper ? hi[i] : lo[i];
-    lo[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
-  }
-}
-
-template <int G> struct Log2 { static constexpr int v = 1 + Log2<G / 2>::v; };
-template <> struct Log2<1> { static constexpr int v = 0; };
-
-// ------------------------------------------------------------------ the photo kernel
-//
-// grid = (n_hyp, n_chunks): blockIdx.x (fastest) is the hypothesis, so CTAs that run together
-// sweep the SAME chunk of (spatially sorted) anchors under different poses and the union of their
-// footprints is a narrow band of the map that stays in L2.
-template <class T, int G, bool CEN>
-__global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_constant__ PassArgs A);
-
-template <class T, int G, bool CEN>
-__device__ __forceinline__ void photo_accumulate(const PassArgs& A, const HypState* st, int chunk_idx,
-                                                 float (&acc)[kNacc]) {
-  constexpr int LOG = Log2<G>::v;
-  const LevelArgs& L = A.lv;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int sub = lane & (G - 1);
-  const unsigned esz = 16 / T::kVec;
-  const unsigned px_stride = (unsigned)L.C * esz;
-  const unsigned row_stride = px_stride * (unsigned)L.W;
-  const char* feat = static_cast<const char*>(L.feat);
-  const char* refb = static_cast<const char*>(L.ref);
-
-  // candidate pose (the pose this pass evaluates), double for the projection
-  double R[9], Cc[3];
-#pragma unroll
-  for (int i = 0; i < 9; ++i) R[i] = st->Rc[i];
-#pragma unroll
-  for (int i = 0; i < 3; ++i) Cc[i] = st->Cc[i];
-
-  const int begin = chunk_idx * A.chunk;
-  const int end = min(begin + A.chunk, L.N);
-  const float wmax = (float)(L.W - 1), hmax = (float)(L.H - 1);
-
-  for (int base = begin + warp * 32; base < end; base += kWarps * 32) {
-    // ---- lane-per-unit: projection + visibility (a2), in double so that u,v carry no fp32 noise
-    const int j = base + lane;
-    bool valid = j < end;
-    float4 P = valid ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, 0.f);
-    double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
-    double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
-    double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
-    double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
-    valid = valid && (Zd > (double)A.prm.z_near);
-    double izd = 1.0 / Zd;
-    double ud = (double)L.fx * Xd * izd + (double)L.cx;
-    double vd = (double)L.fy * Yd * izd + (double)L.cy;
-    double x0d = floor(ud), y0d = floor(vd);
-    valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= (double)wmax) && (y0d + 1.0 <= (double)hmax);
-    float a = valid ? (float)(ud - x0d) : 0.f;
-    float b = valid ? (float)(vd - y0d) : 0.f;
-    int x0 = valid ? (int)x0d : 0, y0 = valid ? (int)y0d : 0;
-    unsigned off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * px_stride;   // invalid units read pixel (0,0)
-    unsigned offv = valid ? off : 0xffffffffu;
-
-    // ---- group rounds: gather + per-unit contraction (a3-a5), reduce-scatter so that lane i ends
-    //      up with the six sums of unit i of this batch
-    float stash[LOG > 0 ? LOG : 1][6];
-    float cur[6];
-    const int gbase = base + (lane & ~(G - 1));           // first unit of this lane's group
-    auto fetch = [&](int r, float& ra, float& rb, bool& rvalid) {
-      unsigned o = __shfl_sync(0xffffffffu, offv, r, G);
-      ra = __shfl_sync(0xffffffffu, a, r, G);
-      rb = __shfl_sync(0xffffffffu, b, r, G);
-      rvalid = o != 0xffffffffu;
-      int jr = min(gbase + r, L.N - 1);
-      return load_taps<16 * G>(feat, (rvalid ? o : 0u) + (unsigned)sub * 16u, row_stride,
-                       refb + ((size_t)jr * L.C) * esz + (size_t)sub * 16u);
-    };
-    float na, nb; bool nvalid;
-    RawTaps nxt;
-    unsigned cflags = 0;                                   // CEN: which outer taps are clamped at the border
-    if constexpr (CEN) cflags = (x0 > 0 ? 1u : 0u) | (x0 + 2 <= L.W - 1 ? 2u : 0u) | (y0 > 0 ? 4u : 0u) | (y0 + 2 <= L.H - 1 ? 8u : 0u);
-    else nxt = fetch(0, na, nb, nvalid);
-#pragma unroll
-    for (int r = 0; r < G; ++r) {
-      bool rvalid;
-      if constexpr (CEN) {
-        unsigned o = __shfl_sync(0xffffffffu, offv, r, G);
-        float ra = __shfl_sync(0xffffffffu, a, r, G), rb = __shfl_sync(0xffffffffu, b, r, G);
-        unsigned fl = __shfl_sync(0xffffffffu, cflags, r, G);
-        rvalid = o != 0xffffffffu;
-        if (!rvalid) fl = 0;                               // invisible units read around pixel (0,0), unclamped side only
-        OuterTaps ot{(fl & 1u) ? -(int)(16 * G) : 0, (fl & 2u) ? 2 * 16 * G : 16 * G,
-                     (fl & 4u) ? -(int)row_stride : 0, (fl & 8u) ? 2 * (int)row_stride : (int)row_stride};
-        int jr = min(gbase + r, L.N - 1);
-        unit_partials_central<T, 16 * G>(feat + (rvalid ? o : 0u) + (unsigned)sub * 16u, row_stride, ot,
-                                         refb + ((size_t)jr * L.C) * esz + (size_t)sub * 16u, ra, rb, cur);
-      } else {
-        RawTaps t = nxt;
-        float ra = na, rb = nb;
-        rvalid = nvalid;
-        if (r + 1 < G) nxt = fetch(r + 1, na, nb, nvalid);   // software pipeline: next unit's loads in flight
-        unit_partials<T>(t, ra, rb, cur);
-      }
-      if (!rvalid) {
-#pragma unroll
-        for (int i = 0; i < 6; ++i) cur[i] = 0.f;
-      }
-#pragma unroll
-      for (int k = 0; k < LOG; ++k) {
-        if (((r >> k) & 1) == 0) {
-#pragma unroll
-          for (int i = 0; i < 6; ++i) stash[k][i] = cur[i];
-          break;
-        }
-        halve<6>(stash[k], cur, 1 << k, (sub >> k) & 1);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) cur[i] = stash[k][i];
-      }
-    }
-
-    // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
-    if (valid) {
-      float wq = 1.f;
-      if (L.conf) {
-        const float* q = L.conf + (size_t)y0 * L.W + x0;
-        float q00 = __ldg(q), q10 = __ldg(q + 1), q01 = __ldg(q + L.W), q11 = __ldg(q + L.W + 1);
-        wq = (1.f - b) * ((1.f - a) * q00 + a * q10) + b * ((1.f - a) * q01 + a * q11);
-      }
-      float w = P.w * wq;
-      float rho, drho;
-      robust<float>(A.prm.loss, w * cur[5], A.prm.loss_scale, rho, drho);
-      float om = w * drho;
-      float X = (float)Xd, Y = (float)Yd, iz = (float)izd;
-      float x = X * iz, y = Y * iz;
-      float fxz = L.fx * iz, fyz = L.fy * iz;
-      // Juv rows (d(u,v)/d(rho,phi)); Ju[1] = Jv[0] = 0
-      float Ju[6] = {fxz, 0.f, -fxz * x, -L.fx * x * y, L.fx * (1.f + x * x), -L.fx * y};
-      float Jv[6] = {0.f, fyz, -fyz * y, -L.fy * (1.f + y * y), L.fy * x * y, L.fy * x};
-      float A11 = om * cur[0], A12 = om * cur[1], A22 = om * cur[2];
-      float b1 = om * cur[3], b2 = om * cur[4];
-#pragma unroll
-      for (int p = 0; p < 6; ++p) {
-        float mu = A11 * Ju[p] + A12 * Jv[p];
-        float mv = A12 * Ju[p] + A22 * Jv[p];
-#pragma unroll
-        for (int q = p; q < 6; ++q) acc[tri(p, q)] += mu * Ju[q] + mv * Jv[q];
-        acc[21 + p] += b1 * Ju[p] + b2 * Jv[p];
-      }
-      acc[27] += rho;
-      acc[28] += 1.f;
-    }
-  }
-}
-
-}  // namespace
-
-namespace {
-
-// ------------------------------------------------------------------ priors (a7, a8), executed by one full warp in double
-
-struct DsmView { const float* d; int w, h; double ox, oy, gsd; };
-
-// Bilinear heightfield sample and exact gradient (per metre). false = outside the DSM.
-__device__ __forceinline__ bool dsm_sample(const DsmView& D, double x, double y, double& z, double& zx, double& zy) {
-  double gx = (x - D.ox) / D.gsd, gy = (y - D.oy) / D.gsd;
-  double fx0 = floor(gx), fy0 = floor(gy);
-  if (!(fx0 >= 0.0) || !(fy0 >= 0.0) || !(fx0 <= (double)(D.w - 2)) || !(fy0 <= (double)(D.h - 2))) return false;
-  int ix = (int)fx0, iy = (int)fy0;
-  double a = gx - fx0, b = gy - fy0;
-  const float* p = D.d + (size_t)iy * D.w + ix;
-  double d00 = __ldg(p), d10 = __ldg(p + 1), d01 = __ldg(p + D.w), d11 = __ldg(p + D.w + 1);
-  z = (1 - b) * ((1 - a) * d00 + a * d10) + b * ((1 - a) * d01 + a * d11);
-  zx = ((1 - b) * (d10 - d00) + b * (d11 - d01)) / D.gsd;
-  zy = ((1 - a) * (d01 - d00) + a * (d11 - d10)) / D.gsd;
-  return true;
-}
-
-__device__ __forceinline__ double height_above(const DsmView& D, const double* C, const double* w, double t) {
-  double z, zx, zy;
-  if (!dsm_sample(D, C[0] + t * w[0], C[1] + t * w[1], z, zx, zy)) return INFINITY;  // off the map = above
-  return C[2] + t * w[2] - z;
-}
-
-// Range residual and 1x6 Jacobian at pose (R_cw, C). Warp-collective (all 32 lanes call it with the same
-// arguments); the 64 march samples are evaluated 32 at a time, one per lane. Result is warp-uniform.
-__device__ bool range_prior(const PassArgs& A, const double* R, const double* C, int lane, double& res, double (&J)[6]) {
-  DsmView D{A.dsm, A.dsm_w, A.dsm_h, (double)A.dsm_ox, (double)A.dsm_oy, (double)A.dsm_gsd};
-  double v[3] = {(double)A.ray[0], (double)A.ray[1], (double)A.ray[2]};
-  double w[3];
-#pragma unroll
-  for (int i = 0; i < 3; ++i) w[i] = R[i] * v[0] + R[3 + i] * v[1] + R[6 + i] * v[2];   // R_cw^T v
-  const double dm = (double)A.range_meas;
-  double dist;
-  if (A.prm.range_mode == PILOT_RANGE_HEIGHT) {
-    dist = dm;
-  } else {
-    const int steps = A.prm.march_steps;
-    const double dt = (double)A.prm.march_tfar_scale * dm / (double)steps;
-    int found = -1;
-    for (int i0 = 0; i0 < steps && found < 0; i0 += 32) {
-      int i = i0 + lane;
-      double f0 = height_above(D, C, w, (double)i * dt);
-      double f1 = height_above(D, C, w, (double)(i + 1) * dt);
-      unsigned hit = __ballot_sync(0xffffffffu, i < steps && f0 > 0.0 && f1 <= 0.0);
-      if (hit) found = i0 + __ffs(hit) - 1;
-    }
-    if (found < 0) return false;
-    double lo = (double)found * dt, hi = (double)(found + 1) * dt;
-    for (int k = 0; k < A.prm.bisect_steps; ++k) {
-      double mid = 0.5 * (lo + hi);
-      if (height_above(D, C, w, mid) > 0.0) lo = mid; else hi = mid;
-    }
-    double flo = height_above(D, C, w, lo), fhi = height_above(D, C, w, hi);
-    if (isfinite(flo) && isfinite(fhi) && flo - fhi > 0.0) dist = lo + (hi - lo) * flo / (flo - fhi);  // secant
-    else dist = hi;
-  }
-  double z, zx, zy;
-  double Pw[3] = {C[0] + dist * w[0], C[1] + dist * w[1], C[2] + dist * w[2]};           // Eq.(5)
-  if (!dsm_sample(D, Pw[0], Pw[1], z, zx, zy)) return false;
-  double n[3] = {-zx, -zy, 1.0};
-  double ndw = 1.0;
-  if (A.prm.range_mode == PILOT_RANGE_HEIGHT) {
-    res = Pw[2] - z;                                                                     // Eq.(6)
-  } else {
-    res = dist - dm;
-    ndw = n[0] * w[0] + n[1] * w[1] + n[2] * w[2];
-    if (!(fabs(ndw) > 1e-12)) return false;
-  }
-  // row = n^T R_cw^T [ -I | [q]x ],  q = dist * v
-  double m[3], q[3] = {dist * v[0], dist * v[1], dist * v[2]};
-#pragma unroll
-  for (int i = 0; i < 3; ++i) m[i] = R[3 * i] * n[0] + R[3 * i + 1] * n[1] + R[3 * i + 2] * n[2];
-  J[0] = -m[0]; J[1] = -m[1]; J[2] = -m[2];
-  J[3] = m[1] * q[2] - m[2] * q[1];      // (m^T [q]x)_0
-  J[4] = m[2] * q[0] - m[0] * q[2];
-  J[5] = m[0] * q[1] - m[1] * q[0];
-  if (A.prm.range_mode == PILOT_RANGE_MARCH) {
-#pragma unroll
-    for (int i = 0; i < 6; ++i) J[i] = -J[i] / ndw;
-  }
-  return true;
-}
-
-// ------------------------------------------------------------------ 6x6 Cholesky solve, SE(3) retraction (a9, a10)
-
-__device__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6]) {
-  double Lm[6][6];
-#pragma unroll
-  for (int i = 0; i < 6; ++i) {
-#pragma unroll
-    for (int j = 0; j <= i; ++j) {
-      double s = Hs[tri(j, i)];
-      if (i == j) s += (damp_mode == PILOT_DAMP_IDENTITY) ? lambda : lambda * fmax(Hs[tri(i, i)], 1e-12);
-#pragma unroll
-      for (int k = 0; k < j; ++k) s -= Lm[i][k] * Lm[j][k];
-      if (i == j) {
-        if (!(s > 0.0) || !isfinite(s)) return false;
-        Lm[i][i] = sqrt(s);
-      } else {
-        Lm[i][j] = s / Lm[j][j];
-      }
-    }
-  }
-  double y[6];
-#pragma unroll
-  for (int i = 0; i < 6; ++i) {
-    double s = g[i];
-#pragma unroll
-    for (int k = 0; k < i; ++k) s -= Lm[i][k] * y[k];
-    y[i] = s / Lm[i][i];
-  }
-#pragma unroll
-  for (int i = 5; i >= 0; --i) {
-    double s = y[i];
-#pragma unroll
-    for (int k = i + 1; k < 6; ++k) s -= Lm[k][i] * x[k];
-    x[i] = s / Lm[i][i];
-  }
-  bool ok = true;
-#pragma unroll
-  for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
-  return ok;
-}
-
-// T_cw <- exp(xi) T_cw (Eq.9): R' = E R, C' = C - R^T E^T V rho
-__device__ void retract(const double* R, const double* C, const double (&xi)[6], double* Rn, double* Cn) {
-  const double px = xi[3], py = xi[4], pz = xi[5];
-  double th2 = px * px + py * py + pz * pz, th = sqrt(th2);
-  double a, b, c;
-  if (th < 1e-4) {
-    a = 1.0 - th2 / 6.0 + th2 * th2 / 120.0;
-    b = 0.5 - th2 / 24.0 + th2 * th2 / 720.0;
-    c = 1.0 / 6.0 - th2 / 120.0 + th2 * th2 / 5040.0;
-  } else {
-    a = sin(th) / th; b = (1.0 - cos(th)) / th2; c = (th - sin(th)) / (th2 * th);
-  }
-  double K[9] = {0, -pz, py, pz, 0, -px, -py, px, 0}, K2[9], E[9], V[9];
-  for (int i = 0; i < 3; ++i)
-    for (int j = 0; j < 3; ++j) K2[3 * i + j] = K[3 * i] * K[j] + K[3 * i + 1] * K[3 + j] + K[3 * i + 2] * K[6 + j];
-  for (int i = 0; i < 9; ++i) {
-    double I = (i % 4 == 0) ? 1.0 : 0.0;
-    E[i] = I + a * K[i] + b * K2[i];
-    V[i] = I + b * K[i] + c * K2[i];
-  }
-  double Vr[3], EtVr[3], Rt[9];
-  for (int i = 0; i < 3; ++i) Vr[i] = V[3 * i] * xi[0] + V[3 * i + 1] * xi[1] + V[3 * i + 2] * xi[2];
-  for (int i = 0; i < 3; ++i) EtVr[i] = E[i] * Vr[0] + E[3 + i] * Vr[1] + E[6 + i] * Vr[2];
-  for (int i = 0; i < 3; ++i)
-    for (int j = 0; j < 3; ++j) Rt[3 * i + j] = E[3 * i] * R[j] + E[3 * i + 1] * R[3 + j] + E[3 * i + 2] * R[6 + j];
-  for (int i = 0; i < 3; ++i) Cn[i] = C[i] - (R[i] * EtVr[0] + R[3 + i] * EtVr[1] + R[6 + i] * EtVr[2]);
-  for (int i = 0; i < 9; ++i) Rn[i] = Rt[i];
-}
-
-}  // namespace
-
-namespace {
-
-// ------------------------------------------------------------------ per-hypothesis finalisation (a6-a11), one warp
-
-__device__ void write_final(const PassArgs& A, const HypState& s, int m) {
-  if (A.out.poses_dev) {
-    float* T = A.out.poses_dev + 12 * (size_t)m;
-    for (int i = 0; i < 3; ++i) {
-      for (int k = 0; k < 3; ++k) T[4 * i + k] = (float)s.R[3 * k + i];     // R_wc = R_cw^T
-      T[4 * i + 3] = (float)s.C[i];
-    }
-  }
-  if (A.out.cost_dev) A.out.cost_dev[m] = (float)s.cost;
-  if (A.out.n_valid_dev) A.out.n_valid_dev[m] = s.n_valid;
-  if (A.out.status_dev) A.out.status_dev[m] = s.status | s.flags;
-}
-
-__device__ void finalize_hypothesis(const PassArgs& A, int m, const float* sums /* smem, kNacc */, int lane) {
-  HypState& s = A.state[m];
-  const pilot_refine_params& P = A.prm;
-
-  // range prior at the evaluated pose: warp-collective
-  double rr = 0.0, Jr[6];
-  bool range_on = P.range_mode != PILOT_RANGE_OFF && P.w_range > 0.f && A.dsm != nullptr;
-  bool range_ok = false;
-  if (range_on) range_ok = range_prior(A, s.Rc, s.Cc, lane, rr, Jr);
-  if (lane != 0) return;
-
-  double Hn[21], gn[6], costn;
-  unsigned fl = 0;
-  for (int i = 0; i < 21; ++i) Hn[i] = (double)sums[i];
-  for (int i = 0; i < 6; ++i) gn[i] = (double)sums[21 + i];
-  costn = (double)sums[27];
-  int nv = (int)(sums[28] + 0.5f);
-  if (nv < P.min_valid) { costn = INFINITY; fl |= PILOT_STATUS_FEW_VALID; }
-
-  if (P.w_gravity > 0.f) {                                                   // Eq.(3)
-    double e[3], r[3];
-    for (int i = 0; i < 3; ++i) {
-      e[i] = s.Rc[3 * i] * (double)A.gw[0] + s.Rc[3 * i + 1] * (double)A.gw[1] + s.Rc[3 * i + 2] * (double)A.gw[2];
-      r[i] = e[i] - (double)A.gi[i];
-    }
-    double rho, drho;
-    robust<double>(P.loss, r[0] * r[0] + r[1] * r[1] + r[2] * r[2], (double)P.gravity_scale, rho, drho);
-    double wg = (double)P.w_gravity * drho;
-    // J = [0 | -[e]x]; rows of -[e]x: (0, e2, -e1), (-e2, 0, e0), (e1, -e0, 0)
-    double Jg[3][3] = {{0, e[2], -e[1]}, {-e[2], 0, e[0]}, {e[1], -e[0], 0}};
-    for (int a = 0; a < 3; ++a) {
-      double ga = 0;
-      for (int i = 0; i < 3; ++i) ga += Jg[i][a] * r[i];
-      gn[3 + a] += wg * ga;
-      for (int b = a; b < 3; ++b) {
-        double h = 0;
-        for (int i = 0; i < 3; ++i) h += Jg[i][a] * Jg[i][b];
-        Hn[tri(3 + a, 3 + b)] += wg * h;
-      }
-    }
-    costn += (double)P.w_gravity * rho;
-  }
-  if (range_on) {                                                            // Eq.(5)-(6) / ray-march
-    if (range_ok) {
-      double rho, drho;
-      robust<double>(P.loss, rr * rr, (double)P.range_scale, rho, drho);
-      double wr = (double)P.w_range * drho;
-      for (int a = 0; a < 6; ++a) {
-        gn[a] += wr * Jr[a] * rr;
-        for (int b = a; b < 6; ++b) Hn[tri(a, b)] += wr * Jr[a] * Jr[b];
-      }
-      costn += (double)P.w_range * rho;
-    } else {
-      fl |= PILOT_STATUS_RANGE_SKIP;
-    }
-  }
-  if (isnan(costn)) s.status |= PILOT_STATUS_NONFINITE;
-
-  // accept / reject (a10). The first evaluation of a level is taken unconditionally.
-  double lam = s.lambda;
-  const bool first = s.pending == 0;
-  if (first || P.lm_mode == PILOT_LM_FIXED || costn < s.cost) {
-    for (int i = 0; i < 9; ++i) s.R[i] = s.Rc[i];
-    for (int i = 0; i < 3; ++i) s.C[i] = s.Cc[i];
-    for (int i = 0; i < 21; ++i) s.H[i] = Hn[i];
-    for (int i = 0; i < 6; ++i) s.g[i] = gn[i];
-    s.cost = costn; s.n_valid = nv; s.flags = fl;
-    if (!first && P.lm_mode == PILOT_LM_ADAPTIVE) lam = fmax(lam * (double)P.lambda_down, (double)P.lambda_min);
-  } else {
-    lam = fmin(lam * (double)P.lambda_up, (double)P.lambda_max);
-  }
-
-  // record + damped solve (a9, Eq.8); a failed factorisation consumes the iteration and raises lambda
-  bool have = false;
-  const size_t Hn_ = (size_t)A.n_hyp;
-  while (s.k < A.iters) {
-    const size_t ri = (size_t)(A.rec_base + s.k) * Hn_ + (size_t)m;
-    if (A.out.iter_hessian_dev) {
-      float* o = A.out.iter_hessian_dev + 36 * ri;
-      for (int a = 0; a < 6; ++a)
-        for (int b = 0; b < 6; ++b) o[6 * a + b] = (float)s.H[a <= b ? tri(a, b) : tri(b, a)];
-    }
-    if (A.out.iter_gradient_dev) for (int a = 0; a < 6; ++a) A.out.iter_gradient_dev[6 * ri + a] = (float)s.g[a];
-    if (A.out.iter_cost_dev) A.out.iter_cost_dev[ri] = (float)s.cost;
-    if (A.out.iter_lambda_dev) A.out.iter_lambda_dev[ri] = (float)lam;
-    double dxi[6];
-    bool ok = chol_solve6(s.H, lam, P.damp_mode, s.g, dxi);
-    s.k += 1;
-    if (ok) {
-      for (int i = 0; i < 6; ++i) dxi[i] = -dxi[i];
-      retract(s.R, s.C, dxi, s.Rc, s.Cc);                                    // Eq.(9)
-      s.pending = 1;
-      have = true;
-      break;
-    }
-    if (lam >= (double)P.lambda_max) s.status |= PILOT_STATUS_CHOL_FAIL;
-    lam = fmin(lam * (double)P.lambda_up, (double)P.lambda_max);
-  }
-  s.lambda = lam;
-  if (!have) {                                                               // this level is finished
-    s.level = A.level + 1;
-    s.k = 0; s.pending = 0; s.lambda = (double)P.lambda_init;
-    for (int i = 0; i < 9; ++i) s.Rc[i] = s.R[i];
-    for (int i = 0; i < 3; ++i) s.Cc[i] = s.C[i];
-    if (A.level + 1 == A.level_end) write_final(A, s, m);
-  }
-}
-
 // ------------------------------------------------------------------ kernels
 
 template <class T, int G, bool CEN>
-__global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_constant__ PassArgs A) {
+__global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
   const int m = blockIdx.x, chunk_idx = blockIdx.y;
   const HypState* st = A.state + m;
   if (st->level != A.level) return;             // finished this level early (failed factorisations)
 
-  float acc[kNacc];
-#pragma unroll
-  for (int i = 0; i < kNacc; ++i) acc[i] = 0.f;
-  photo_accumulate<T, G, CEN>(A, st, chunk_idx, acc);
+  PILOT_DECLARE_ACC
+  PILOT_ZERO_ACC
+  {
+    const int begin = chunk_idx * A.chunk;
+    photo_accumulate<T, G, CEN>(A, st->Rc, st->Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc);
+  }
+  PILOT_LOAD_ACC
 
   // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -727,7 +70,7 @@ __global__ void __launch_bounds__(kThreads) photo_pass_kernel(const __grid_const
   s_sum[lane] = t;
   if (lane == 0) A.counters[m] = 0u;
   __syncwarp();
-  finalize_hypothesis(A, m, s_sum, lane);
+  finalize_hypothesis(A, A.state[m], m, s_sum, lane, nullptr);
 }
 
 __global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init,
@@ -761,6 +104,8 @@ struct pilot_refine_handle {
   bool owns_ws;
   int max_chunks;
   int chunk_override;       // 0 = heuristic
+  int mode;                 // pilot_exec_mode
+  int cluster_override;     // 0 = heuristic
   int sm_count;
   int last_launches;
   // host-path staging (create_host only)
@@ -835,6 +180,19 @@ pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode) {
   return grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(d, g) : pick_t<false>(d, g);
 }
 
+// Small problems (few (anchor, hypothesis) units per level) are launch- and tail-latency bound with one launch per
+// pass: they go to the cluster-resident kernel, one launch per level. Returns the cluster size, 0 = pass kernel.
+int choose_resident(const pilot_refine_handle* h, int n_hyp, int n_points) {
+  if (h->mode == PILOT_EXEC_PASSES) return 0;
+  // AUTO: resident only when every hypothesis' cluster is co-resident in one wave (2 CTAs per SM) and the level is small
+  if (h->mode == PILOT_EXEC_AUTO && ((long)n_hyp * (long)n_points > 1500000L || n_hyp > 2 * h->sm_count)) return 0;
+  if (h->cluster_override > 0) return h->cluster_override;
+  // as many CTAs per hypothesis as keep the whole set co-resident (2 CTAs per SM) with about one batch per warp
+  int s = 8;
+  while (s > 1 && ((long)n_hyp * s > 2L * h->sm_count || n_points / s < 200)) s >>= 1;
+  return s;
+}
+
 int choose_chunk(const pilot_refine_handle* h, int n_hyp, int n_points) {
   if (h->chunk_override > 0) return h->chunk_override;
   // enough CTAs for ~4 waves at 2 CTAs/SM, chunks of 256..2048 anchors
@@ -869,6 +227,8 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->cfg = *cfg;
   h->max_chunks = w.max_chunks;
   h->chunk_override = 0;
+  h->mode = PILOT_EXEC_AUTO;
+  h->cluster_override = 0;
   h->last_launches = 0;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
   cudaDeviceProp prop;
@@ -906,6 +266,14 @@ int pilot_refine_destroy(pilot_refine_handle* h) {
 int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk) {
   if (!h || chunk < 0 || (chunk % kMinChunk) != 0) return PILOT_ERR_ARG;
   h->chunk_override = chunk;
+  return PILOT_OK;
+}
+
+int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster) {
+  if (!h || mode < PILOT_EXEC_AUTO || mode > PILOT_EXEC_RESIDENT) return PILOT_ERR_ARG;
+  if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return PILOT_ERR_ARG;
+  h->mode = mode;
+  h->cluster_override = cluster;
   return PILOT_OK;
 }
 
@@ -979,12 +347,22 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     A.chunk = choose_chunk(h, A.n_hyp, L.N);
     A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
     if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
-    pass_fn fn = pick_kernel(c.feat_dtype, lanes_per_unit(L.C, c.feat_dtype), p->grad_mode);
-    dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
-    for (int pass = 0; pass <= p->iters[l]; ++pass) {
-      A.pass = pass;
-      fn<<<grid, kThreads, 0, st>>>(A);
+    const int g = lanes_per_unit(L.C, c.feat_dtype);
+    const int cluster = choose_resident(h, A.n_hyp, L.N);
+    if (cluster > 0) {
+      if (resident_launch(c.feat_dtype, g, p->grad_mode, A, cluster, cuda_stream) != (int)cudaSuccess) {
+        if (prev != c.device) cudaSetDevice(prev);
+        return PILOT_ERR_CUDA;
+      }
       ++launches;
+    } else {
+      pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode);
+      dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
+      for (int pass = 0; pass <= p->iters[l]; ++pass) {
+        A.pass = pass;
+        fn<<<grid, kThreads, 0, st>>>(A);
+        ++launches;
+      }
     }
     rec_base += p->iters[l];
   }

@@ -1,0 +1,187 @@
+// pilot_resident.cu — the cluster-resident LM kernel for small problems (latency-bound regime: the paper's own
+// frame shape of 10^2-10^3 hypotheses x 500 anchors; BASELINE configs 0, 1, 3).
+//
+// One launch per pyramid LEVEL instead of one per EVAL pass: a thread-block cluster of S CTAs owns one hypothesis
+// for all of that level's LM iterations (hypotheses are independent, so clusters never wait on each other).
+// Per iteration: every CTA gathers its slice of the anchors (same photo_accumulate as the pass kernel), reduces it
+// to 32 floats in shared memory; after a cluster barrier the rank-0 CTA sums the S slices through distributed
+// shared memory in a fixed order (deterministic), adds the priors, takes the accept/reject decision, solves the
+// damped 6x6 system and retracts (finalize_hypothesis, shared with the pass kernel); a second cluster barrier
+// publishes the new candidate pose, which the other CTAs read from rank 0's shared memory. The heightfield
+// ray-march of the range prior depends only on the candidate pose, so one warp of the rank-0 CTA evaluates it
+// WHILE the other warps gather: it leaves the critical path. The optimiser state lives in shared memory for the
+// whole level; launches, grid ramps, the atomic ticket and the global partial sums of the pass kernel disappear.
+//
+// Shares no code with oracle/.
+#include "pilot_device.cuh"
+
+#include <cooperative_groups.h>
+#include <string.h>
+
+namespace cg = cooperative_groups;
+
+namespace {
+
+struct ResidentShared {
+  HypState st;                       // rank 0: the hypothesis' optimiser state for the whole level
+  double pose[12];                   // this CTA's copy of the candidate pose: Rc[9], Cc[3]
+  float part[kWarps][kNacc];
+  float cta_sum[kNacc];              // this CTA's slice total; rank 0 reads it through DSMEM
+  float tot[kNacc];
+  PriorRes prior;
+  int go;
+};
+
+template <class T, int G, bool CEN>
+__global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel(const __grid_constant__ PassArgs A) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const unsigned S = cluster.num_blocks(), rank = cluster.block_rank();
+  const int m = (int)(blockIdx.x / S);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __shared__ ResidentShared sh;
+  PILOT_DECLARE_ACC
+
+  if (rank == 0) {
+    const int* src = reinterpret_cast<const int*>(A.state + m);
+    int* dst = reinterpret_cast<int*>(&sh.st);
+    for (int i = threadIdx.x; i < (int)(sizeof(HypState) / 4); i += kThreads) dst[i] = src[i];
+    __syncthreads();
+    if (threadIdx.x == 0) sh.go = sh.st.level == A.level;
+  }
+  const ResidentShared* master = cluster.map_shared_rank(&sh, 0);
+  const bool range_on = range_enabled(A);
+  const bool prior_warp = range_on && rank == 0 && warp == kWarps - 1;
+  const int n_workers = (range_on && rank == 0) ? kWarps - 1 : kWarps;
+  const int N = A.lv.N;
+  const int per = (((N + (int)S - 1) / (int)S) + 31) / 32 * 32;      // anchors per CTA, whole 32-unit batches
+  const int begin = min((int)rank * per, N), end = min(begin + per, N);
+
+#ifdef PILOT_RESIDENT_PROFILE
+  long long t_eval = 0, t_fin = 0, t_red = 0, t_all = clock64(), t0 = 0, n_it = 0;
+#endif
+  for (;;) {
+    cluster.sync();                                  // rank 0's candidate pose and go flag are published
+#ifdef PILOT_RESIDENT_PROFILE
+    t0 = clock64();
+#endif
+    const int go = master->go;
+    if (threadIdx.x < 12) sh.pose[threadIdx.x] = threadIdx.x < 9 ? master->st.Rc[threadIdx.x] : master->st.Cc[threadIdx.x - 9];
+    __syncthreads();
+    if (!go) break;
+
+    PILOT_ZERO_ACC
+    if (prior_warp) {
+      double rr = 0.0, Jr[6];
+      const bool ok = range_prior(A, sh.pose, sh.pose + 9, lane, rr, Jr);
+      if (lane == 0) {
+        sh.prior.ok = ok ? 1 : 0; sh.prior.r = rr;
+        for (int i = 0; i < 6; ++i) sh.prior.J[i] = ok ? Jr[i] : 0.0;
+      }
+    } else {
+      photo_accumulate<T, G, CEN>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc);
+    }
+    PILOT_LOAD_ACC
+#ifdef PILOT_RESIDENT_PROFILE
+    t_eval += clock64() - t0; t0 = clock64();
+#endif
+    // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
+#pragma unroll
+    for (int half = 16; half >= 1; half >>= 1) {
+      const bool upper = lane & half;
+#pragma unroll
+      for (int i = 0; i < half; ++i) {
+        float send = upper ? acc[i] : acc[i + half];
+        float keep = upper ? acc[i + half] : acc[i];
+        acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+      }
+    }
+    sh.part[warp][lane] = acc[0];
+    __syncthreads();
+    if (warp == 0) {
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) t += sh.part[w][lane];            // fixed order
+      sh.cta_sum[lane] = t;
+    }
+    cluster.sync();                                  // every slice total (and the prior) is in shared memory
+#ifdef PILOT_RESIDENT_PROFILE
+    t_red += clock64() - t0; t0 = clock64(); ++n_it;
+#endif
+    if (rank == 0 && warp == 0) {
+      float v[8];
+#pragma unroll
+      for (unsigned r = 0; r < 8; ++r) v[r] = r < S ? cluster.map_shared_rank(&sh, r)->cta_sum[lane] : 0.f;   // loads in flight together
+      float t = 0.f;
+#pragma unroll
+      for (unsigned r = 0; r < 8; ++r) t += v[r];                         // fixed order
+      sh.tot[lane] = t;
+      __syncwarp();
+      finalize_hypothesis(A, sh.st, m, sh.tot, lane, range_on ? &sh.prior : nullptr);
+      __syncwarp();
+      if (lane == 0) sh.go = sh.st.level == A.level;
+#ifdef PILOT_RESIDENT_PROFILE
+      t_fin += clock64() - t0;
+#endif
+    }
+  }
+#ifdef PILOT_RESIDENT_PROFILE
+  if (rank == 0 && (threadIdx.x == 0 || threadIdx.x == kThreads - 1 || threadIdx.x == 32)) {
+    float* o = A.partials + (size_t)m * 32 + (threadIdx.x == 0 ? 0 : (threadIdx.x == 32 ? 8 : 16));
+    o[0] = (float)t_eval; o[1] = (float)t_red; o[2] = (float)t_fin; o[3] = (float)(clock64() - t_all); o[4] = (float)n_it;
+  }
+#endif
+  if (rank == 0) {                                   // the state goes back to the workspace for the next level
+    const int* src = reinterpret_cast<const int*>(&sh.st);
+    int* dst = reinterpret_cast<int*>(A.state + m);
+    for (int i = threadIdx.x; i < (int)(sizeof(HypState) / 4); i += kThreads) dst[i] = src[i];
+  }
+  cluster.sync();                                    // rank 0's shared memory outlives every remote read
+}
+
+typedef void (*resident_fn)(const PassArgs);
+
+template <class T, bool CEN>
+resident_fn pick_g(int g) {
+  switch (g) {
+    case 1: return lm_resident_kernel<T, 1, CEN>;
+    case 2: return lm_resident_kernel<T, 2, CEN>;
+    case 4: return lm_resident_kernel<T, 4, CEN>;
+    case 8: return lm_resident_kernel<T, 8, CEN>;
+    case 16: return lm_resident_kernel<T, 16, CEN>;
+    case 32: return lm_resident_kernel<T, 32, CEN>;
+  }
+  return nullptr;
+}
+
+template <bool CEN>
+resident_fn pick_t(pilot_dtype d, int g) {
+  switch (d) {
+    case PILOT_F32: return pick_g<F32Tag, CEN>(g);
+    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
+    case PILOT_F16: return pick_g<F16Tag, CEN>(g);
+  }
+  return nullptr;
+}
+
+}  // namespace
+
+int pilot_internal::resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, const PassArgs& A, int cluster,
+                                    void* stream) {
+  resident_fn fn = grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(dtype, lanes_per_unit)
+                                                           : pick_t<false>(dtype, lanes_per_unit);
+  if (!fn || cluster < 1 || cluster > 8 || (cluster & (cluster - 1))) return (int)cudaErrorInvalidValue;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof cfg);
+  cfg.gridDim = dim3((unsigned)A.n_hyp * (unsigned)cluster, 1, 1);
+  cfg.blockDim = dim3(kThreads, 1, 1);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = static_cast<cudaStream_t>(stream);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cluster;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return (int)cudaLaunchKernelEx(&cfg, fn, A);
+}

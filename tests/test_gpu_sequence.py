@@ -43,7 +43,7 @@ def test_config3_streaming_sequence():
             nxt = next(gen)
             S.upload(nxt)                      # frame i+1 copies while frame i refines
         S.step(seq.params)
-        assert S.last_launches == 1 + sum(k + 1 for k in seq.iters) + 3
+        assert S.last_launches == 1 + 3 + 3            # AUTO: one cluster-resident launch per level at this size
         if i in checked:
             kept[i] = cur
             gpu_sets[i] = S.last_frame()       # synchronises: test only
@@ -67,8 +67,9 @@ def test_config3_streaming_sequence():
         assert abs(int(rows[i, 14]) - orc["n_valid"][gb]) <= 2
         assert rows[i, 12] == gpu_sets[i][2].min() and gpu_sets[i][2][gb] == rows[i, 12]
         assert gb == int(np.argmin(gpu_sets[i][2]))
-        # the GPU seeds are the oracle's to fp32 rounding
-        assert np.abs(gpu_sets[i][0] - seeds).max() <= 4e-5
+        # frame 0: the same prior on both sides, so the GPU seeds are the oracle's to fp32 rounding; later frames are
+        # seeded from each side's own previous estimate, which agree to the pose tolerance
+        assert np.abs(gpu_sets[i][0] - seeds).max() <= (4e-5 if i == 0 else 2 * TOL)
         prior = orc["poses64"][b].astype(np.float32).astype(np.float64)     # the estimate crosses the API as fp32
 
     # ---- every 50th frame: the oracle refines the GPU's own seeds of that frame
