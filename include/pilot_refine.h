@@ -302,6 +302,39 @@ int pilot_refine_sequence_last_launches(const pilot_refine_sequence* s);
 int pilot_refine_sequence_destroy(pilot_refine_sequence* s);
 
 /* ---------------------------------------------------------------------------------------------
+ * Reference-crop geometry that produces the geo-anchors (supp II-B). Asynchronous on
+ * `cuda_stream`, no allocation, no host synchronisation. The heightfield arguments are those of
+ * pilot_refine_inputs (dsm_dev [dsm_height][dsm_width] fp32, origin, metres per sample).
+ */
+
+/*
+ * Map-footprint estimation, supp Eq.(2): rays from the camera centre of pose_dev ([12] row-major
+ * [R_wc | C]) through the image corners (0,0), (W-1,0), (W-1,H-1), (0,H-1) of a width x height image with
+ * intrinsics (fx, fy, cx, cy); along each ray the sample s_i = i*s_max/n_samples, i = 1..n_samples, with the smallest
+ * |z_ray(s) - h_DSM(x_ray(s), y_ray(s))| (bilinear h_DSM; samples outside the heightfield are skipped; ties -> the
+ * smallest s). corners_dev[4][4] = x, y, z_ray at s*, and that residual; a ray with no sample over the heightfield
+ * gives a row of NaN. Decisions are taken in double precision.
+ */
+int pilot_refine_footprint(const float* pose_dev, const float intrinsics[4], int width, int height,
+                           const float* dsm_dev, int dsm_width, int dsm_height,
+                           float dsm_origin_x, float dsm_origin_y, float dsm_gsd,
+                           int n_samples, float s_max, float* corners_dev, void* cuda_stream);
+
+/*
+ * Pixel-aligned warping + geo-anchor construction, supp Eq.(3): the homography that maps the
+ * crop corners (0,0), (Wc-1,0), (Wc-1,Hc-1), (0,Hc-1) onto the footprint corners_dev[4][4] (x, y used) gives every
+ * crop pixel pix_dev[n][2] = (u, v) its map coordinates (x^m, y^m); the warped DSM layer D^r is the bilinear
+ * heightfield sample there. points_dev[n][4] = x^m, y^m, D^r, w with w = 1, or (x^m, y^m, 0, 0) when the pixel falls
+ * outside the heightfield or the footprint is degenerate — the layout pilot_refine_inputs.points_dev takes (an
+ * anchor of weight 0 contributes nothing to Eq.2).
+ */
+int pilot_refine_lift_anchors(const float* corners_dev, int crop_width, int crop_height,
+                              const float* pix_dev, int n,
+                              const float* dsm_dev, int dsm_width, int dsm_height,
+                              float dsm_origin_x, float dsm_origin_y, float dsm_gsd,
+                              float* points_dev, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Measurement helper: random-gather bandwidth of this GPU with the photo kernel's access
  * shape — aligned reads of vec_bytes (16..512, power of two; vec_bytes/16 lanes x 16-byte ld.global.nc) at
  * hashed positions of a buffer of buffer_bytes (e.g. 16 MiB = L2-resident, 1 GiB = HBM). Allocates and frees

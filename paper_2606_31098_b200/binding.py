@@ -30,7 +30,8 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_select_best", "pilot_refine_prune_topk",
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
-           "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather"]
+           "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
+           "pilot_refine_footprint", "pilot_refine_lift_anchors"]
 SEQ_ROW = 16
 
 
@@ -145,6 +146,12 @@ def lib():
         L.pilot_refine_sequence_last_frame.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.pilot_refine_sequence_last_launches.argtypes = [C.c_void_p]
         L.pilot_refine_sequence_destroy.argtypes = [C.c_void_p]
+        L.pilot_refine_footprint.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_int,
+                                             C.c_float, C.c_float, C.c_float, C.c_int, C.c_float, C.c_void_p, C.c_void_p]
+        L.pilot_refine_footprint.restype = C.c_int
+        L.pilot_refine_lift_anchors.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int,
+                                                C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
+        L.pilot_refine_lift_anchors.restype = C.c_int
         L.pilot_refine_probe_gather.argtypes = [C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.pilot_refine_probe_gather.restype = C.c_int
         for name in EXPORTS:
@@ -591,3 +598,31 @@ def probe_gather(buffer_bytes, vec_bytes, launches=5, device=0):
     _check(lib().pilot_refine_probe_gather(int(device), int(buffer_bytes), int(vec_bytes), int(launches), C.byref(g)),
            "pilot_refine_probe_gather")
     return g.value
+
+
+# ------------------------------------------------------------------ reference-crop geometry (supp II-B)
+
+def footprint(pose, intrinsics, width, height, dsm, dsm_origin, dsm_gsd, n_samples, s_max, stream=None):
+    """supp Eq.(2). pose: cuda float32 [12]; dsm: cuda float32 [Hd, Wd]. -> cuda float32 [4, 4] (x, y, z, residual)."""
+    torch = _torch()
+    assert pose.is_cuda and dsm.is_cuda and pose.dtype == dsm.dtype == torch.float32 and dsm.is_contiguous()
+    K = (C.c_float * 4)(*[float(k) for k in intrinsics])
+    out = torch.empty(4, 4, dtype=torch.float32, device=pose.device)
+    _check(lib().pilot_refine_footprint(pose.data_ptr(), K, int(width), int(height), dsm.data_ptr(), dsm.shape[1],
+                                        dsm.shape[0], float(dsm_origin[0]), float(dsm_origin[1]), float(dsm_gsd),
+                                        int(n_samples), float(s_max), out.data_ptr(),
+                                        _stream_ptr(torch, stream, pose.device)), "pilot_refine_footprint")
+    return out
+
+
+def lift_anchors(corners, crop_w, crop_h, pix, dsm, dsm_origin, dsm_gsd, stream=None):
+    """supp Eq.(3). corners: cuda float32 [4, 4]; pix: cuda float32 [n, 2] crop pixels -> anchors cuda float32 [n, 4]."""
+    torch = _torch()
+    assert corners.is_cuda and pix.is_cuda and pix.dtype == torch.float32 and pix.is_contiguous() and dsm.is_contiguous()
+    n = int(pix.shape[0])
+    out = torch.empty(n, 4, dtype=torch.float32, device=pix.device)
+    _check(lib().pilot_refine_lift_anchors(corners.data_ptr(), int(crop_w), int(crop_h), pix.data_ptr(), n,
+                                           dsm.data_ptr(), dsm.shape[1], dsm.shape[0], float(dsm_origin[0]),
+                                           float(dsm_origin[1]), float(dsm_gsd), out.data_ptr(),
+                                           _stream_ptr(torch, stream, pix.device)), "pilot_refine_lift_anchors")
+    return out
