@@ -97,6 +97,42 @@ __device__ __forceinline__ uint4 ldg16(const void* p) {
   return __ldg(reinterpret_cast<const uint4*>(p));
 }
 
+// ------------------------------------------------------------------ fast double reciprocal / reciprocal sqrt
+//
+// A double-precision divide or sqrt is a ~30-instruction dependent sequence; the per-hypothesis finalisation (one
+// lane, the serial tail of every LM iteration) and the ray-march are chains of them. These start from the fp32
+// hardware approximation and take two Newton steps in double (relative error ~1e-16 inside the fp32 range).
+__device__ __forceinline__ double inv_sqrt(double s) {
+  if (!(s > 1e-30) || !(s < 1e30)) return 1.0 / sqrt(s);
+  double y = (double)rsqrtf((float)s);
+  y = y * (1.5 - 0.5 * s * y * y);
+  y = y * (1.5 - 0.5 * s * y * y);
+  return y;
+}
+__device__ __forceinline__ double fast_rcp(double d) {
+  const double ad = fabs(d);
+  if (!(ad > 1e-30) || !(ad < 1e30)) return 1.0 / d;
+  double y = (double)__frcp_rn((float)d);
+  y = y * (2.0 - d * y);
+  y = y * (2.0 - d * y);
+  return y;
+}
+
+// rho, rho' for the prior terms, in double, without sqrt / divide
+__device__ __forceinline__ void robust_d(int loss, double x, double scale, double& rho, double& drho) {
+  rho = x; drho = 1.0;
+  if (scale > 0.0) {
+    const double s2 = scale * scale;
+    if (loss == PILOT_LOSS_HUBER) {
+      if (x > s2) { const double y = inv_sqrt(x); rho = 2.0 * scale * (x * y) - s2; drho = scale * y; }
+    } else if (loss == PILOT_LOSS_CAUCHY) {
+      const double q = x * fast_rcp(s2);
+      rho = s2 * log1p(q);
+      drho = fast_rcp(1.0 + q);
+    }
+  }
+}
+
 // ------------------------------------------------------------------ robust loss (Eq.2 / Eq.7)
 
 template <typename T>
@@ -308,7 +344,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
     double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
     double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
     valid = valid && (Zd > (double)A.prm.z_near);
-    double izd = 1.0 / Zd;
+    double izd = fast_rcp(Zd);
     double ud = (double)L.fx * Xd * izd + (double)L.cx;
     double vd = (double)L.fy * Yd * izd + (double)L.cy;
     double x0d = floor(ud), y0d = floor(vd);
@@ -432,11 +468,18 @@ namespace {
 
 // ------------------------------------------------------------------ priors (a7, a8), executed by one full warp in double
 
-struct DsmView { const float* d; int w, h; double ox, oy, gsd; };
+struct DsmView { const float* d; int w, h; double ox, oy, gsd, ig; };   // ig = 1 / gsd
+__host__ __device__ inline DsmView make_dsm_view(const float* d, int w, int h, float ox, float oy, float gsd) {
+#ifdef __CUDA_ARCH__
+  return DsmView{d, w, h, (double)ox, (double)oy, (double)gsd, fast_rcp((double)gsd)};
+#else
+  return DsmView{d, w, h, (double)ox, (double)oy, (double)gsd, 1.0 / (double)gsd};
+#endif
+}
 
 // Bilinear heightfield sample and exact gradient (per metre). false = outside the DSM.
 __device__ __forceinline__ bool dsm_sample(const DsmView& D, double x, double y, double& z, double& zx, double& zy) {
-  double gx = (x - D.ox) / D.gsd, gy = (y - D.oy) / D.gsd;
+  double gx = (x - D.ox) * D.ig, gy = (y - D.oy) * D.ig;
   double fx0 = floor(gx), fy0 = floor(gy);
   if (!(fx0 >= 0.0) || !(fy0 >= 0.0) || !(fx0 <= (double)(D.w - 2)) || !(fy0 <= (double)(D.h - 2))) return false;
   int ix = (int)fx0, iy = (int)fy0;
@@ -444,8 +487,8 @@ __device__ __forceinline__ bool dsm_sample(const DsmView& D, double x, double y,
   const float* p = D.d + (size_t)iy * D.w + ix;
   double d00 = __ldg(p), d10 = __ldg(p + 1), d01 = __ldg(p + D.w), d11 = __ldg(p + D.w + 1);
   z = (1 - b) * ((1 - a) * d00 + a * d10) + b * ((1 - a) * d01 + a * d11);
-  zx = ((1 - b) * (d10 - d00) + b * (d11 - d01)) / D.gsd;
-  zy = ((1 - a) * (d01 - d00) + a * (d11 - d10)) / D.gsd;
+  zx = ((1 - b) * (d10 - d00) + b * (d11 - d01)) * D.ig;
+  zy = ((1 - a) * (d01 - d00) + a * (d11 - d10)) * D.ig;
   return true;
 }
 
@@ -458,7 +501,7 @@ __device__ __forceinline__ double height_above(const DsmView& D, const double* C
 // Range residual and 1x6 Jacobian at pose (R_cw, C). Warp-collective (all 32 lanes call it with the same
 // arguments); the 64 march samples are evaluated 32 at a time, one per lane. Result is warp-uniform.
 __device__ bool range_prior(const PassArgs& A, const double* R, const double* C, int lane, double& res, double (&J)[6]) {
-  DsmView D{A.dsm, A.dsm_w, A.dsm_h, (double)A.dsm_ox, (double)A.dsm_oy, (double)A.dsm_gsd};
+  const DsmView D = make_dsm_view(A.dsm, A.dsm_w, A.dsm_h, A.dsm_ox, A.dsm_oy, A.dsm_gsd);
   double v[3] = {(double)A.ray[0], (double)A.ray[1], (double)A.ray[2]};
   double w[3];
 #pragma unroll
@@ -485,7 +528,7 @@ __device__ bool range_prior(const PassArgs& A, const double* R, const double* C,
       if (height_above(D, C, w, mid) > 0.0) lo = mid; else hi = mid;
     }
     double flo = height_above(D, C, w, lo), fhi = height_above(D, C, w, hi);
-    if (isfinite(flo) && isfinite(fhi) && flo - fhi > 0.0) dist = lo + (hi - lo) * flo / (flo - fhi);  // secant
+    if (isfinite(flo) && isfinite(fhi) && flo - fhi > 0.0) dist = lo + (hi - lo) * flo * fast_rcp(flo - fhi);  // secant
     else dist = hi;
   }
   double z, zx, zy;
@@ -510,23 +553,14 @@ __device__ bool range_prior(const PassArgs& A, const double* R, const double* C,
   J[5] = m[0] * q[1] - m[1] * q[0];
   if (A.prm.range_mode == PILOT_RANGE_MARCH) {
 #pragma unroll
-    for (int i = 0; i < 6; ++i) J[i] = -J[i] / ndw;
+    const double indw = fast_rcp(ndw);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) J[i] = -J[i] * indw;
   }
   return true;
 }
 
 // ------------------------------------------------------------------ 6x6 Cholesky solve, SE(3) retraction (a9, a10)
-
-// 1/sqrt(s) in double from the fp32 hardware approximation + two Newton steps (relative error ~1e-16): a
-// double-precision sqrt or divide is a ~30-instruction dependent sequence, and this solve sits on the serial tail of
-// every LM iteration, so the factorisation keeps only reciprocals of the pivots.
-__device__ __forceinline__ double inv_sqrt(double s) {
-  if (!(s > 1e-30) || !(s < 1e30)) return 1.0 / sqrt(s);
-  double y = (double)rsqrtf((float)s);
-  y = y * (1.5 - 0.5 * s * y * y);
-  y = y * (1.5 - 0.5 * s * y * y);
-  return y;
-}
 
 __device__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6]) {
   double Lm[6][6], inv[6];
@@ -571,14 +605,27 @@ __device__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode
 // T_cw <- exp(xi) T_cw (Eq.9): R' = E R, C' = C - R^T E^T V rho
 __device__ void retract(const double* R, const double* C, const double (&xi)[6], double* Rn, double* Cn) {
   const double px = xi[3], py = xi[4], pz = xi[5];
-  double th2 = px * px + py * py + pz * pz, th = sqrt(th2);
-  double a, b, c;
-  if (th < 1e-4) {
-    a = 1.0 - th2 / 6.0 + th2 * th2 / 120.0;
-    b = 0.5 - th2 / 24.0 + th2 * th2 / 720.0;
-    c = 1.0 / 6.0 - th2 / 120.0 + th2 * th2 / 5040.0;
+  const double th2 = px * px + py * py + pz * pz;
+  double a, b, c;      // sin(th)/th, (1 - cos th)/th^2, (th - sin th)/th^3: even power series in th
+  if (th2 <= 0.25) {
+    // LM steps are small rotations: 10 terms of the series (next term < 3e-23 at th = 0.5) instead of sqrt/sin/cos
+    constexpr double f[22] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
+                              1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0,
+                              1.0 / 87178291200.0, 1.0 / 1307674368000.0, 1.0 / 20922789888000.0,
+                              1.0 / 355687428096000.0, 1.0 / 6402373705728000.0, 1.0 / 121645100408832000.0,
+                              1.0 / 2432902008176640000.0, 1.0 / 51090942171709440000.0};
+    a = f[19]; b = f[20]; c = f[21];
+#pragma unroll
+    for (int k = 8; k >= 0; --k) {
+      a = f[2 * k + 1] - th2 * a;
+      b = f[2 * k + 2] - th2 * b;
+      c = f[2 * k + 3] - th2 * c;
+    }
   } else {
-    a = sin(th) / th; b = (1.0 - cos(th)) / th2; c = (th - sin(th)) / (th2 * th);
+    const double th = sqrt(th2);
+    double sn, cs;
+    sincos(th, &sn, &cs);
+    a = sn / th; b = (1.0 - cs) / th2; c = (th - sn) / (th2 * th);
   }
   double K[9] = {0, -pz, py, pz, 0, -px, -py, px, 0}, K2[9], E[9], V[9];
   for (int i = 0; i < 3; ++i)
@@ -641,6 +688,12 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     }
   }
   if (lane != 0) return;
+#ifdef PILOT_FIN_PROFILE
+  long long tp[6]; tp[0] = clock64();
+#define PILOT_TP(i) tp[i] = clock64();
+#else
+#define PILOT_TP(i)
+#endif
 
   double Hn[21], gn[6], costn;
   unsigned fl = 0;
@@ -657,7 +710,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
       r[i] = e[i] - (double)A.gi[i];
     }
     double rho, drho;
-    robust<double>(P.loss, r[0] * r[0] + r[1] * r[1] + r[2] * r[2], (double)P.gravity_scale, rho, drho);
+    robust_d(P.loss, r[0] * r[0] + r[1] * r[1] + r[2] * r[2], (double)P.gravity_scale, rho, drho);
     double wg = (double)P.w_gravity * drho;
     // J = [0 | -[e]x]; rows of -[e]x: (0, e2, -e1), (-e2, 0, e0), (e1, -e0, 0)
     double Jg[3][3] = {{0, e[2], -e[1]}, {-e[2], 0, e[0]}, {e[1], -e[0], 0}};
@@ -676,7 +729,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
   if (range_on) {                                                            // Eq.(5)-(6) / ray-march
     if (range_ok) {
       double rho, drho;
-      robust<double>(P.loss, rr * rr, (double)P.range_scale, rho, drho);
+      robust_d(P.loss, rr * rr, (double)P.range_scale, rho, drho);
       double wr = (double)P.w_range * drho;
       for (int a = 0; a < 6; ++a) {
         gn[a] += wr * Jr[a] * rr;
@@ -688,6 +741,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     }
   }
   if (isnan(costn)) s.status |= PILOT_STATUS_NONFINITE;
+  PILOT_TP(1)
 
   // accept / reject (a10). The first evaluation of a level is taken unconditionally.
   double lam = s.lambda;
@@ -703,6 +757,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     lam = fmin(lam * (double)P.lambda_up, (double)P.lambda_max);
   }
 
+  PILOT_TP(2)
   // record + damped solve (a9, Eq.8); a failed factorisation consumes the iteration and raises lambda
   bool have = false;
   const size_t Hn_ = (size_t)A.n_hyp;
@@ -717,11 +772,14 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     if (A.out.iter_cost_dev) A.out.iter_cost_dev[ri] = (float)s.cost;
     if (A.out.iter_lambda_dev) A.out.iter_lambda_dev[ri] = (float)lam;
     double dxi[6];
+    PILOT_TP(3)
     bool ok = chol_solve6(s.H, lam, P.damp_mode, s.g, dxi);
+    PILOT_TP(4)
     s.k += 1;
     if (ok) {
       for (int i = 0; i < 6; ++i) dxi[i] = -dxi[i];
       retract(s.R, s.C, dxi, s.Rc, s.Cc);                                    // Eq.(9)
+      PILOT_TP(5)
       s.pending = 1;
       have = true;
       break;
@@ -737,6 +795,10 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     for (int i = 0; i < 3; ++i) s.Cc[i] = s.C[i];
     if (A.level + 1 == A.level_end) write_final(A, s, m);
   }
+#ifdef PILOT_FIN_PROFILE
+  if (have) { float* o = A.partials + (size_t)m * 32 + 24; for (int i = 0; i < 5; ++i) o[i] += (float)(tp[i + 1] - tp[i]); o[5] += 1.f; }
+#endif
+#undef PILOT_TP
 }
 
 }  // namespace

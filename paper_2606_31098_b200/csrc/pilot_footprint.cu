@@ -113,7 +113,7 @@ int pilot_refine_footprint(const float* pose_dev, const float intrinsics[4], int
   if (!pose_dev || !intrinsics || !corners_dev || width < 2 || height < 2 || n_samples < 1 || !(s_max > 0.f) ||
       !(intrinsics[0] > 0.f) || !(intrinsics[1] > 0.f) || !dsm_ok(dsm_dev, dsm_width, dsm_height, dsm_gsd))
     return PILOT_ERR_ARG;
-  DsmView D{dsm_dev, dsm_width, dsm_height, (double)dsm_origin_x, (double)dsm_origin_y, (double)dsm_gsd};
+  const DsmView D = make_dsm_view(dsm_dev, dsm_width, dsm_height, dsm_origin_x, dsm_origin_y, dsm_gsd);
   footprint_kernel<<<1, 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(pose_dev, intrinsics[0], intrinsics[1], intrinsics[2],
                                                                           intrinsics[3], width, height, D, n_samples,
                                                                           (double)s_max, corners_dev);
@@ -126,7 +126,7 @@ int pilot_refine_lift_anchors(const float* corners_dev, int crop_width, int crop
   if (n < 0 || crop_width < 2 || crop_height < 2 || !dsm_ok(dsm_dev, dsm_width, dsm_height, dsm_gsd)) return PILOT_ERR_ARG;
   if (n == 0) return PILOT_OK;
   if (!corners_dev || !pix_dev || !points_dev || ((uintptr_t)points_dev & 15)) return PILOT_ERR_ARG;
-  DsmView D{dsm_dev, dsm_width, dsm_height, (double)dsm_origin_x, (double)dsm_origin_y, (double)dsm_gsd};
+  const DsmView D = make_dsm_view(dsm_dev, dsm_width, dsm_height, dsm_origin_x, dsm_origin_y, dsm_gsd);
   lift_kernel<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(corners_dev, crop_width, crop_height,
                                                                                   pix_dev, n, D, points_dev);
   return cudaGetLastError() == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
