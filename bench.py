@@ -400,7 +400,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="config4", choices=sorted(WORKLOADS))
     ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA of the pass kernel (0 = heuristic)")
-    ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident"], help="launch strategy (pilot_exec_mode)")
+    ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident", "split"], help="launch strategy (pilot_exec_mode)")
     ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -471,6 +471,17 @@ def main():
                 "note": "4*C*s gather bytes per (anchor,hypothesis) unit x H*N units per launch (north_star's "
                         "HBM-gather roofline, no-reuse model); the taps are served through L2, so achieved may "
                         "exceed the HBM copy peak when L2 reuse is high"}
+    # the bound that actually applies: plain fp32 arithmetic. Algorithmic flops per unit-evaluation =
+    # 2*(19*C + 120); peak = SMs x 128 fp32 lanes x 2 flop x max SM clock
+    prop = torch.cuda.get_device_properties(local_rank)
+    flops_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2)) \
+        * 2 * (19 * W.prob["channels"][-1] + 120)
+    alu_peak = prop.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
+    roofline["alu"] = {"bound": "alu", "achieved": flops_per_launch / launch_s / 1e12, "peak": alu_peak,
+                       "unit": "TFLOP/s", "frac": flops_per_launch / launch_s / 1e12 / alu_peak,
+                       "note": "fp32 FMA lanes: 2*(19*C+120) algorithmic flop per unit-evaluation against "
+                               "SMs*128*2*1.965 GHz; the kernel is issue/FMA-pipe bound, not byte bound "
+                               "(profiles/r1b_photo_config4.md)"}
     if rank == 0 and not args.no_probe:
         # the build's own micro-benchmark: random gathers with the kernel's access shape
         tap = 4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2) // 4      # one tap = one pixel

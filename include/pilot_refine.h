@@ -169,10 +169,13 @@ int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk);
  * Launch strategy. PASSES: one launch per EVAL pass, (hypothesis x anchor-chunk) CTAs — the throughput path for
  * large hypothesis x anchor products. RESIDENT: one launch per pyramid level, a thread-block cluster of `cluster`
  * CTAs (1, 2, 4, 8; 0 = heuristic) owns a hypothesis for all of the level's LM iterations — the latency path for
- * small problems (the paper's own frame shape). AUTO (default) picks per level by H x N. Both compute the same
+ * small problems (the paper's own frame shape). PASSES_SPLIT: as PASSES, but the per-hypothesis finalisation (priors,
+ * accept/reject, solve, update) runs in a second launch with one warp per hypothesis instead of in the last CTA of
+ * each hypothesis — for many hypotheses with few anchors each (the 1210-hypothesis coarse level). AUTO (default)
+ * picks per level from H, N and the SM count. All compute the same
  * sums from the same per-unit arithmetic; they differ in fp32 summation order only.
  */
-typedef enum { PILOT_EXEC_AUTO = 0, PILOT_EXEC_PASSES = 1, PILOT_EXEC_RESIDENT = 2 } pilot_exec_mode;
+typedef enum { PILOT_EXEC_AUTO = 0, PILOT_EXEC_PASSES = 1, PILOT_EXEC_RESIDENT = 2, PILOT_EXEC_PASSES_SPLIT = 3 } pilot_exec_mode;
 int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster);
 
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */

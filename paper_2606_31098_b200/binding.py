@@ -21,7 +21,7 @@ GRAD_CODE = {"bilinear_exact": 0, "central_sampled": 1}
 ERRORS = {-1: "bad argument", -2: "workspace too small", -3: "unsupported shape / mode", -4: "CUDA error"}
 
 SEED_CODE = {"camera": 0, "world": 1}
-EXEC_CODE = {"auto": 0, "passes": 1, "resident": 2}
+EXEC_CODE = {"auto": 0, "passes": 1, "resident": 2, "split": 3}
 TOPK_MAX = 8192
 
 EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy",

@@ -72,6 +72,7 @@ struct PassArgs {
   // run
   int n_hyp, level, level_end, pass, iters, rec_base;
   int chunk, n_chunks;
+  int defer;                // 1: the pass kernel only writes partial sums; finalize_kernel ends the iteration
   HypState* state;
   float* partials;          // [n_hyp][n_chunks][kNacc]
   unsigned* counters;       // [n_hyp]
@@ -799,6 +800,23 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
   if (have) { float* o = A.partials + (size_t)m * 32 + 24; for (int i = 0; i < 5; ++i) o[i] += (float)(tp[i + 1] - tp[i]); o[5] += 1.f; }
 #endif
 #undef PILOT_TP
+}
+
+// The same on the state in the workspace (global memory): lane 0 works on a private copy, so that the optimiser
+// state sits in registers / L1 instead of being re-read from L2 around every output store. Warp-collective.
+__device__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane) {
+  HypState loc;
+  const HypState& g = A.state[m];
+  if (lane == 0) {
+    loc = g;
+  } else {                       // the other lanes only need the candidate pose (ray-march of the range prior)
+#pragma unroll
+    for (int i = 0; i < 9; ++i) loc.Rc[i] = g.Rc[i];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) loc.Cc[i] = g.Cc[i];
+  }
+  finalize_hypothesis(A, loc, m, sums, lane, nullptr);
+  if (lane == 0) A.state[m] = loc;
 }
 
 }  // namespace

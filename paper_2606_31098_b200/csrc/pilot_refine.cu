@@ -55,10 +55,12 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) t += s_part[w][lane];                    // fixed order
     A.partials[((size_t)m * A.n_chunks + chunk_idx) * kNacc + lane] = t;
+    if (A.defer) return;                         // finalize_kernel (next launch) ends the iteration
     __threadfence();
     __syncwarp();
     if (lane == 0) s_last = (atomicAdd(A.counters + m, 1u) == (unsigned)(A.n_chunks - 1));
   }
+  if (A.defer) return;
   __syncthreads();
   if (!s_last || warp != 0) return;
 
@@ -70,7 +72,24 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   s_sum[lane] = t;
   if (lane == 0) A.counters[m] = 0u;
   __syncwarp();
-  finalize_hypothesis(A, A.state[m], m, s_sum, lane, nullptr);
+  finalize_in_workspace(A, m, s_sum, lane);
+}
+
+// Deferred finalisation: one WARP per hypothesis. With many hypotheses and few anchors each (the paper's coarse level:
+// 1210 x 500) every CTA of the pass kernel would end in the serial fp64 tail while holding an SM slot that waiting CTAs
+// need; here all hypotheses finalise side by side instead.
+constexpr int kFinWarps = 4;
+__global__ void __launch_bounds__(kFinWarps * 32) finalize_kernel(const __grid_constant__ PassArgs A) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int m = blockIdx.x * kFinWarps + warp;
+  __shared__ float s_sum[kFinWarps][kNacc];
+  if (m >= A.n_hyp || A.state[m].level != A.level) return;
+  float t = 0.f;
+  const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
+  for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);      // fixed order
+  s_sum[warp][lane] = t;
+  __syncwarp();
+  finalize_in_workspace(A, m, s_sum[warp], lane);
 }
 
 __global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init,
@@ -183,7 +202,7 @@ pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode) {
 // Small problems (few (anchor, hypothesis) units per level) are launch- and tail-latency bound with one launch per
 // pass: they go to the cluster-resident kernel, one launch per level. Returns the cluster size, 0 = pass kernel.
 int choose_resident(const pilot_refine_handle* h, int n_hyp, int n_points) {
-  if (h->mode == PILOT_EXEC_PASSES) return 0;
+  if (h->mode == PILOT_EXEC_PASSES || h->mode == PILOT_EXEC_PASSES_SPLIT) return 0;
   // AUTO: resident only when every hypothesis' cluster is co-resident in one wave (2 CTAs per SM) and the level is small
   if (h->mode == PILOT_EXEC_AUTO && ((long)n_hyp * (long)n_points > 1500000L || n_hyp > 2 * h->sm_count)) return 0;
   if (h->cluster_override > 0) return h->cluster_override;
@@ -270,7 +289,7 @@ int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk) {
 }
 
 int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster) {
-  if (!h || mode < PILOT_EXEC_AUTO || mode > PILOT_EXEC_RESIDENT) return PILOT_ERR_ARG;
+  if (!h || mode < PILOT_EXEC_AUTO || mode > PILOT_EXEC_PASSES_SPLIT) return PILOT_ERR_ARG;
   if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return PILOT_ERR_ARG;
   h->mode = mode;
   h->cluster_override = cluster;
@@ -358,11 +377,22 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     } else {
       pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode);
       dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
+      // small CTAs (<= 512 anchors) in more than one wave, or many hypotheses (measured: config 2, H = 1024, -4 %):
+      // the serial tail moves to its own launch
+      const int per_cta = A.chunk < L.N ? A.chunk : L.N;
+      A.defer = h->mode == PILOT_EXEC_PASSES_SPLIT ||
+                (h->mode == PILOT_EXEC_AUTO &&
+                 ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 512));
       for (int pass = 0; pass <= p->iters[l]; ++pass) {
         A.pass = pass;
         fn<<<grid, kThreads, 0, st>>>(A);
         ++launches;
+        if (A.defer) {
+          finalize_kernel<<<(A.n_hyp + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(A);
+          ++launches;
+        }
       }
+      A.defer = 0;
     }
     rec_base += p->iters[l];
   }

@@ -145,9 +145,9 @@ def test_paper_schedule_1210_to_128():
     torch.cuda.synchronize()
     g = {k: v.cpu().numpy() for k, v in out.items()}
     it = prob["params"]["iters"]
-    # AUTO: 1210 hypotheses do not fit one wave of clusters -> one launch per pass on the coarse level;
-    # the 128 kept ones run cluster-resident, one launch per level
-    assert pr.launches == (1 + it[0] + 1) + (1 + 2) + 3
+    # AUTO: 1210 hypotheses do not fit one wave of clusters -> on the coarse level one gather launch + one
+    # finalisation launch per pass; the 128 kept ones run cluster-resident, one launch per level
+    assert pr.launches == (1 + 2 * (it[0] + 1)) + (1 + 2) + 3
     pr.close()
 
     # oracle pipeline (its own seeds from the same fp32 offset table)
