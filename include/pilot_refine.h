@@ -146,7 +146,7 @@ int pilot_refine_destroy(pilot_refine_handle* h);
 /*
  * Host-buffer path (what bench.py's "e2e" times): every "_dev" pointer of `in_host` and
  * `out_host` is a HOST pointer (pinned memory recommended). run_host copies the inputs into
- * device staging owned by the handle (cudaMemcpyAsync on `cuda_stream`), enqueues
+ * device staging owned by the handle (cudaMemcpyAsync on the handle's copy stream), enqueues
  * pilot_refine_run, copies the requested outputs back and synchronises the stream before
  * returning. The staging is sized at create_host() from cfg plus the DSM capacity given
  * there and is allocated once with cudaMalloc (cfg->workspace_dev must be NULL); a run whose
@@ -157,6 +157,20 @@ int pilot_refine_create_host(const pilot_refine_config* cfg, int max_dsm_width, 
 int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in_host,
                           const pilot_refine_params* p, const pilot_refine_outputs* out_host,
                           void* cuda_stream);
+
+/*
+ * The same, pipelined: submit_host() enqueues the upload of one run's inputs on the handle's own copy stream into
+ * one of TWO device staging halves, then — on `cuda_stream`, after an event — the run and the copy of its outputs
+ * to out_host, and returns a ticket (>= 0) at once; wait_host() blocks until the OLDEST submitted run's outputs are
+ * in host memory. Submitting run k+1 before waiting for run k overlaps its upload with run k's kernels. At most two
+ * runs may be in flight (a third submit returns PILOT_ERR_UNSUPPORTED); the host buffers of a run (inputs: pinned
+ * memory, or the upload serialises; outputs) must stay valid until its wait_host() returned.
+ * run_host == submit_host + wait_host.
+ */
+int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in_host,
+                             const pilot_refine_params* p, const pilot_refine_outputs* out_host,
+                             void* cuda_stream);
+int pilot_refine_wait_host(pilot_refine_handle* h);
 
 /*
  * Tuning knob: anchors per CTA of the photo kernel (a multiple of 256; 0 = built-in heuristic,

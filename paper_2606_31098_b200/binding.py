@@ -25,7 +25,8 @@ EXEC_CODE = {"auto": 0, "passes": 1, "resident": 2, "split": 3}
 TOPK_MAX = 8192
 
 EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy",
-           "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_last_launches",
+           "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_submit_host",
+           "pilot_refine_wait_host", "pilot_refine_last_launches",
            "pilot_refine_run_levels", "pilot_refine_set_exec_mode", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
            "pilot_refine_select_best", "pilot_refine_prune_topk",
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
@@ -112,7 +113,9 @@ def lib():
         L.pilot_refine_create.restype = C.c_int
         L.pilot_refine_create_host.argtypes = [C.POINTER(Config), C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         L.pilot_refine_create_host.restype = C.c_int
-        for name in ("pilot_refine_run", "pilot_refine_run_host"):
+        L.pilot_refine_wait_host.argtypes = [C.c_void_p]
+        L.pilot_refine_wait_host.restype = C.c_int
+        for name in ("pilot_refine_run", "pilot_refine_run_host", "pilot_refine_submit_host"):
             fn = getattr(L, name)
             fn.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.POINTER(Outputs), C.c_void_p]
             fn.restype = C.c_int
@@ -285,6 +288,35 @@ class Refiner:
                       iter_gradient=torch.zeros(T * H * 6, dtype=torch.float32, **kw),
                       iter_cost=torch.zeros(T * H, dtype=torch.float32, **kw),
                       iter_lambda=torch.zeros(T * H, dtype=torch.float32, **kw))
+
+    # ---- pipelined host path: submit run k+1 before waiting for run k so that its upload overlaps run k's kernels
+    def submit(self, di, params, stream=None, outputs=("poses", "cost", "n_valid", "status")):
+        assert self.host_path, "submit/wait is the host-buffer path"
+        torch = self.torch
+        if not hasattr(self, "_sets"):
+            self._sets = [self.o, {k: torch.zeros_like(v).pin_memory() for k, v in self.o.items()}]
+            self._pending, self._nsub = [], 0
+        k = self._nsub                                   # host output sets alternate; at most two runs are in flight
+        par, P = make_params(params, di.n_levels)
+        out = Outputs()
+        o = self._sets[k & 1]
+        for name in outputs:
+            setattr(out, name + "_dev", o[name].data_ptr())
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        t = lib().pilot_refine_submit_host(self.handle, C.byref(di.inp), C.byref(par), C.byref(out),
+                                           C.c_void_p(stream.cuda_stream))
+        if t < 0:
+            _check(t, "pilot_refine_submit_host")
+        self._pending.append((k, o, outputs, di.n_hyp, sum(P["iters"])))
+        self._nsub = k + 1
+        return t
+
+    def wait(self):
+        """Blocks until the oldest submitted run's outputs are in (pinned) host memory; returns them (views)."""
+        _check(lib().pilot_refine_wait_host(self.handle), "pilot_refine_wait_host")
+        k, o, outputs, H, T = self._pending.pop(0)
+        return {name: (o[name][:H] if not name.startswith("iter_") else o[name]) for name in outputs}
 
     @classmethod
     def for_inputs(cls, di, params, device=0, host_path=False):

@@ -130,8 +130,11 @@ struct pilot_refine_handle {
   // host-path staging (create_host only)
   bool host_mode;
   int max_dsm_w, max_dsm_h;
-  char* stage;              // one cudaMalloc
+  char* stage;              // one cudaMalloc: two halves of stage_bytes each
   size_t stage_bytes;
+  cudaStream_t copy_stream; // uploads of submit_host
+  cudaEvent_t ev_copied[2], ev_done[2];
+  long n_submitted, n_waited;
 };
 
 namespace {
@@ -250,6 +253,8 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->cluster_override = 0;
   h->last_launches = 0;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
+  h->copy_stream = nullptr; h->n_submitted = h->n_waited = 0;
+  for (int i = 0; i < 2; ++i) { h->ev_copied[i] = nullptr; h->ev_done[i] = nullptr; }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) { delete h; cudaSetDevice(prev); return PILOT_ERR_CUDA; }
   h->sm_count = prop.multiProcessorCount;
@@ -276,6 +281,11 @@ int pilot_refine_destroy(pilot_refine_handle* h) {
   cudaGetDevice(&prev);
   cudaSetDevice(h->cfg.device);
   if (h->owns_ws && h->ws) cudaFree(h->ws);
+  if (h->copy_stream) { cudaStreamSynchronize(h->copy_stream); cudaStreamDestroy(h->copy_stream); }
+  for (int i = 0; i < 2; ++i) {
+    if (h->ev_done[i]) { cudaEventSynchronize(h->ev_done[i]); cudaEventDestroy(h->ev_done[i]); }
+    if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
+  }
   if (h->stage) cudaFree(h->stage);
   cudaSetDevice(prev);
   delete h;
@@ -451,18 +461,24 @@ int pilot_refine_create_host(const pilot_refine_config* cfg, int max_dsm_width, 
   cudaSetDevice(cfg->device);
   StageLayout s = stage_layout(cfg, max_dsm_width, max_dsm_height);
   void* p = nullptr;
-  cudaError_t e = cudaMalloc(&p, s.total);
+  bool ok = cudaMalloc(&p, 2 * s.total) == cudaSuccess;            // two halves: run k+1 uploads while run k computes
+  if (ok) {
+    h->stage = static_cast<char*>(p);
+    h->stage_bytes = s.total;
+    ok = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i)
+      ok = cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming) == cudaSuccess &&
+           cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
+  }
   cudaSetDevice(prev);
-  if (e != cudaSuccess) { pilot_refine_destroy(h); *out = nullptr; return PILOT_ERR_CUDA; }
-  h->stage = static_cast<char*>(p);
-  h->stage_bytes = s.total;
   h->host_mode = true;
   h->max_dsm_w = max_dsm_width; h->max_dsm_h = max_dsm_height;
+  if (!ok) { pilot_refine_destroy(h); *out = nullptr; return PILOT_ERR_CUDA; }
   return PILOT_OK;
 }
 
-int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
-                          const pilot_refine_outputs* out, void* cuda_stream) {
+int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                             const pilot_refine_outputs* out, void* cuda_stream) {
   if (!h || !in || !p || !out || !h->host_mode) return PILOT_ERR_ARG;
   const pilot_refine_config& c = h->cfg;
   if (in->n_hypotheses < 0 || in->n_hypotheses > c.max_hypotheses) return in->n_hypotheses < 0 ? PILOT_ERR_ARG : PILOT_ERR_UNSUPPORTED;
@@ -474,18 +490,22 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in,
   }
   if (T > c.max_total_iters) return PILOT_ERR_UNSUPPORTED;
   if (in->dsm_dev && ((size_t)in->dsm_width * in->dsm_height > (size_t)h->max_dsm_w * h->max_dsm_h)) return PILOT_ERR_UNSUPPORTED;
+  if (h->n_submitted - h->n_waited >= 2) return PILOT_ERR_UNSUPPORTED;      // both halves in flight
   int prev = 0;
   cudaGetDevice(&prev);
   if (prev != c.device && cudaSetDevice(c.device) != cudaSuccess) return PILOT_ERR_CUDA;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int half = (int)(h->n_submitted & 1);
+  char* stage = h->stage + (size_t)half * h->stage_bytes;
   StageLayout s = stage_layout(&c, h->max_dsm_w, h->max_dsm_h);
   size_t es = elem_size(c.feat_dtype), H = (size_t)in->n_hypotheses;
   pilot_refine_inputs din = *in;
   bool ok = true;
+  // the run that last used this half (two submissions ago) has been waited for, so the half is free on the device
   auto up = [&](size_t at, const void* src, size_t bytes) -> void* {
     if (!src || bytes == 0) return nullptr;
-    ok = ok && cudaMemcpyAsync(h->stage + at, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
-    return h->stage + at;
+    ok = ok && cudaMemcpyAsync(stage + at, src, bytes, cudaMemcpyHostToDevice, h->copy_stream) == cudaSuccess;
+    return stage + at;
   };
   for (int l = 0; l < c.n_levels; ++l) {
     size_t px = (size_t)c.width[l] * c.height[l], N = (size_t)in->n_points[l];
@@ -496,15 +516,17 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in,
   }
   din.init_poses_dev = static_cast<const float*>(up(s.poses, in->init_poses_dev, H * 48));
   din.dsm_dev = static_cast<const float*>(up(s.dsm, in->dsm_dev, (size_t)in->dsm_width * in->dsm_height * 4));
+  ok = ok && cudaEventRecord(h->ev_copied[half], h->copy_stream) == cudaSuccess;
+  ok = ok && cudaStreamWaitEvent(st, h->ev_copied[half], 0) == cudaSuccess;
   pilot_refine_outputs dout;
-  dout.poses_dev = out->poses_dev ? reinterpret_cast<float*>(h->stage + s.o_poses) : nullptr;
-  dout.cost_dev = out->cost_dev ? reinterpret_cast<float*>(h->stage + s.o_cost) : nullptr;
-  dout.n_valid_dev = out->n_valid_dev ? reinterpret_cast<int*>(h->stage + s.o_nvalid) : nullptr;
-  dout.status_dev = out->status_dev ? reinterpret_cast<unsigned*>(h->stage + s.o_status) : nullptr;
-  dout.iter_hessian_dev = out->iter_hessian_dev ? reinterpret_cast<float*>(h->stage + s.o_ih) : nullptr;
-  dout.iter_gradient_dev = out->iter_gradient_dev ? reinterpret_cast<float*>(h->stage + s.o_ig) : nullptr;
-  dout.iter_cost_dev = out->iter_cost_dev ? reinterpret_cast<float*>(h->stage + s.o_ic) : nullptr;
-  dout.iter_lambda_dev = out->iter_lambda_dev ? reinterpret_cast<float*>(h->stage + s.o_il) : nullptr;
+  dout.poses_dev = out->poses_dev ? reinterpret_cast<float*>(stage + s.o_poses) : nullptr;
+  dout.cost_dev = out->cost_dev ? reinterpret_cast<float*>(stage + s.o_cost) : nullptr;
+  dout.n_valid_dev = out->n_valid_dev ? reinterpret_cast<int*>(stage + s.o_nvalid) : nullptr;
+  dout.status_dev = out->status_dev ? reinterpret_cast<unsigned*>(stage + s.o_status) : nullptr;
+  dout.iter_hessian_dev = out->iter_hessian_dev ? reinterpret_cast<float*>(stage + s.o_ih) : nullptr;
+  dout.iter_gradient_dev = out->iter_gradient_dev ? reinterpret_cast<float*>(stage + s.o_ig) : nullptr;
+  dout.iter_cost_dev = out->iter_cost_dev ? reinterpret_cast<float*>(stage + s.o_ic) : nullptr;
+  dout.iter_lambda_dev = out->iter_lambda_dev ? reinterpret_cast<float*>(stage + s.o_il) : nullptr;
   int rc = ok ? pilot_refine_run(h, &din, p, &dout, cuda_stream) : PILOT_ERR_CUDA;
   if (rc == PILOT_OK) {
     auto down = [&](void* dst, const void* src, size_t bytes) {
@@ -518,11 +540,33 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in,
     down(out->iter_gradient_dev, dout.iter_gradient_dev, (size_t)T * H * 24);
     down(out->iter_cost_dev, dout.iter_cost_dev, (size_t)T * H * 4);
     down(out->iter_lambda_dev, dout.iter_lambda_dev, (size_t)T * H * 4);
-    ok = ok && cudaStreamSynchronize(st) == cudaSuccess;
+    ok = ok && cudaEventRecord(h->ev_done[half], st) == cudaSuccess;
     if (!ok) rc = PILOT_ERR_CUDA;
   }
   if (prev != c.device) cudaSetDevice(prev);
-  return rc;
+  if (rc != PILOT_OK) return rc;
+  const int ticket = (int)(h->n_submitted & 0x3fffffff);
+  h->n_submitted += 1;
+  return ticket;
+}
+
+int pilot_refine_wait_host(pilot_refine_handle* h) {
+  if (!h || !h->host_mode || h->n_waited >= h->n_submitted) return PILOT_ERR_ARG;
+  const int half = (int)(h->n_waited & 1);
+  h->n_waited += 1;
+  return cudaEventSynchronize(h->ev_done[half]) == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
+}
+
+int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                          const pilot_refine_outputs* out, void* cuda_stream) {
+  if (!h || !h->host_mode) return PILOT_ERR_ARG;
+  while (h->n_waited < h->n_submitted) {                                     // drain anything still in flight
+    int rc = pilot_refine_wait_host(h);
+    if (rc != PILOT_OK) return rc;
+  }
+  int t = pilot_refine_submit_host(h, in, p, out, cuda_stream);
+  if (t < 0) return t;
+  return pilot_refine_wait_host(h);
 }
 
 }  // extern "C"

@@ -275,3 +275,33 @@ def test_run_is_cuda_graph_capturable():
     for k in ("poses", "cost", "iter_hessian", "iter_lambda"):
         assert torch.equal(out[k], eager[k]), k
     r.close()
+
+
+def test_pipelined_host_path_matches_run_host():
+    """submit_host / wait_host with two runs in flight: the same bytes as the synchronous run_host, per run."""
+    from paper_2606_31098_b200 import binding
+    probs = [wl.config1(H=8, N=1000, iters=(2, 2, 2)), wl.config1(H=8, N=1000, iters=(2, 2, 2), idx=7)]
+    his = [binding.DeviceInputs(p, host=True) for p in probs]
+    P = probs[0]["params"]
+    r = binding.Refiner.for_inputs(his[0], P, host_path=True)
+    r.set_exec_mode(MODE["mode"], MODE["cluster"])
+    want = []
+    for hi in his:
+        o = r.run(hi, P)
+        want.append({k: v.clone() for k, v in o.items()})
+    outs = ("poses", "cost", "n_valid", "status", "iter_hessian")
+    r.submit(his[0], P, outputs=outs)
+    r.submit(his[1], P, outputs=outs)
+    with pytest.raises(RuntimeError, match="-3"):
+        r.submit(his[0], P, outputs=outs)              # both halves in flight
+    got = []
+    for k in range(4):                                  # keep two in flight over four runs
+        res = r.wait()
+        got.append({n: v.clone() for n, v in res.items()})
+        if k + 2 < 4:
+            r.submit(his[k % 2], P, outputs=outs)
+    for k in range(4):
+        for n in ("poses", "cost", "n_valid"):
+            assert np.array_equal(got[k][n].numpy(), want[k % 2][n].numpy()), (k, n)
+    assert not np.array_equal(want[0]["poses"].numpy(), want[1]["poses"].numpy())
+    r.close()
