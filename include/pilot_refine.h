@@ -173,7 +173,7 @@ int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* 
 int pilot_refine_wait_host(pilot_refine_handle* h);
 
 /*
- * Tuning knob: anchors per CTA of the photo kernel (a multiple of 256; 0 = built-in heuristic,
+ * Tuning knob: anchors per CTA of the photo kernel (a multiple of 128; 0 = built-in heuristic,
  * which sizes the grid to a few waves of 2 CTAs per SM). Results do not depend on it beyond
  * fp32 summation order.
  */

@@ -23,11 +23,19 @@ namespace {
 #define PILOT_SMEM_ACC 1        // 1: the 29 per-thread accumulators live in shared memory (a [32][256] fp32 array, one
                                 // conflict-free column per thread) so that the registers they held carry prefetched taps
 #endif
+#ifndef PILOT_SMEM_RS
+#define PILOT_SMEM_RS 1         // 1: the per-unit sum over a lane group's channel slices goes through a shared-memory
+                                // transpose (3 STS.64 per round + 1.5 G LDS.128 + 6 (G-1) FADD per batch) instead of the
+                                // shuffle reduce-scatter (6 (G-1) x (SHFL + 2 FSEL + FADD)); used for 2 <= G <= 8
+#endif
 #ifndef PILOT_MIN_BLOCKS
 #define PILOT_MIN_BLOCKS 2      // resident CTAs per SM the kernels are compiled for (register cap 128 / 85)
 #endif
 
-constexpr int kThreads = 256;            // threads per CTA of the photo kernel
+#ifndef PILOT_THREADS
+#define PILOT_THREADS 256
+#endif
+constexpr int kThreads = PILOT_THREADS;   // threads per CTA of the gather kernels
 constexpr int kWarps = kThreads / 32;
 constexpr int kNacc = 32;                // 21 H + 6 g + cost + n_valid, padded to 32 floats
 constexpr int kMinChunk = kWarps * 32;   // one 32-unit batch per warp
@@ -302,6 +310,20 @@ __device__ __forceinline__ void halve(float (&lo)[N], const float (&hi)[N], int 
 template <int G> struct Log2 { static constexpr int v = 1 + Log2<G / 2>::v; };
 template <> struct Log2<1> { static constexpr int v = 0; };
 
+// Shared-memory transpose of the group reduction: row u of a warp's buffer holds, for unit u of the batch, the six
+// partial sums of each of the G lanes ([G][6] floats). Row stride = 6 G rounded up to an odd multiple of 4 words, so
+// that the 32 lanes' LDS.128 of their own rows are conflict-free.
+template <int G> struct RedRows {
+  static constexpr bool kOn = PILOT_SMEM_RS && G >= 2 && G <= 8;
+  static constexpr int kStride = G == 2 ? 12 : (G == 4 ? 28 : (G == 8 ? 52 : 0));
+  static constexpr int kWarpFloats = kOn ? 32 * kStride : 0;
+};
+// dynamic shared memory of the gather kernels: [accumulators kNacc x kThreads] [kWarps reduction buffers]
+inline size_t gather_smem_for(int g);
+template <int G> constexpr size_t gather_smem_bytes() {
+  return (size_t)(PILOT_SMEM_ACC ? kNacc * kThreads : 0) * 4 + (size_t)kWarps * RedRows<G>::kWarpFloats * 4;
+}
+
 // ------------------------------------------------------------------ the photo kernel
 //
 // grid = (n_hyp, n_chunks): blockIdx.x (fastest) is the hypothesis, so CTAs that run together
@@ -310,7 +332,7 @@ template <> struct Log2<1> { static constexpr int v = 0; };
 template <class T, int G, bool CEN>
 __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double* Rc, const double* Ccand,
                                                  int begin, int end, int worker, int n_workers,
-                                                 float (&acc)[kNacc], float* sacc) {
+                                                 float (&acc)[kNacc], float* sacc, float* red /* this warp's rows */) {
 #if PILOT_SMEM_ACC
 #define PILOT_ACC(i) sacc[(i) * kThreads]     // this thread's column of the [kNacc][kThreads] shared array
 #else
@@ -404,17 +426,40 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
 #pragma unroll
         for (int i = 0; i < 6; ++i) cur[i] = 0.f;
       }
+      if constexpr (RedRows<G>::kOn) {
+        float2* row = reinterpret_cast<float2*>(red + ((lane & ~(G - 1)) + r) * RedRows<G>::kStride + sub * 6);
+        row[0] = make_float2(cur[0], cur[1]); row[1] = make_float2(cur[2], cur[3]); row[2] = make_float2(cur[4], cur[5]);
+      } else {
 #pragma unroll
-      for (int k = 0; k < LOG; ++k) {
-        if (((r >> k) & 1) == 0) {
+        for (int k = 0; k < LOG; ++k) {
+          if (((r >> k) & 1) == 0) {
 #pragma unroll
-          for (int i = 0; i < 6; ++i) stash[k][i] = cur[i];
-          break;
+            for (int i = 0; i < 6; ++i) stash[k][i] = cur[i];
+            break;
+          }
+          halve<6>(stash[k], cur, 1 << k, (sub >> k) & 1);
+#pragma unroll
+          for (int i = 0; i < 6; ++i) cur[i] = stash[k][i];
         }
-        halve<6>(stash[k], cur, 1 << k, (sub >> k) & 1);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) cur[i] = stash[k][i];
       }
+    }
+    if constexpr (RedRows<G>::kOn) {                       // lane i sums the G slices of unit i, in lane order
+      __syncwarp();
+      const float4* rp = reinterpret_cast<const float4*>(red + lane * RedRows<G>::kStride);
+      float v[6 * G];
+#pragma unroll
+      for (int i = 0; i < 6 * G / 4; ++i) {
+        float4 t = rp[i];
+        v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+      }
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        float t = v[c];
+#pragma unroll
+        for (int g = 1; g < G; ++g) t += v[6 * g + c];
+        cur[c] = t;
+      }
+      __syncwarp();                                        // rows are rewritten by the next batch
     }
 
     // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
@@ -452,13 +497,28 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
 #undef PILOT_ACC
 }
 
+inline size_t gather_smem_for(int g) {
+  switch (g) {
+    case 1: return gather_smem_bytes<1>();
+    case 2: return gather_smem_bytes<2>();
+    case 4: return gather_smem_bytes<4>();
+    case 8: return gather_smem_bytes<8>();
+    case 16: return gather_smem_bytes<16>();
+    case 32: return gather_smem_bytes<32>();
+  }
+  return 0;
+}
+
 // The per-thread accumulators before / after photo_accumulate (registers, or a column of shared memory).
 #if PILOT_SMEM_ACC
-#define PILOT_DECLARE_ACC __shared__ float s_acc[kNacc * kThreads]; float* sacc = s_acc + threadIdx.x; float acc[kNacc];
+#define PILOT_DECLARE_ACC extern __shared__ float4 pilot_dyn_smem[]; \
+  float* sacc = reinterpret_cast<float*>(pilot_dyn_smem) + threadIdx.x; float acc[kNacc]; \
+  float* red = reinterpret_cast<float*>(pilot_dyn_smem) + kNacc * kThreads + (threadIdx.x >> 5) * RedRows<G>::kWarpFloats;
 #define PILOT_ZERO_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) sacc[i * kThreads] = 0.f;
 #define PILOT_LOAD_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) acc[i] = sacc[i * kThreads];
 #else
-#define PILOT_DECLARE_ACC float* sacc = nullptr; float acc[kNacc];
+#define PILOT_DECLARE_ACC extern __shared__ float4 pilot_dyn_smem[]; float* sacc = nullptr; float acc[kNacc]; \
+  float* red = reinterpret_cast<float*>(pilot_dyn_smem) + (threadIdx.x >> 5) * RedRows<G>::kWarpFloats;
 #define PILOT_ZERO_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) acc[i] = 0.f;
 #define PILOT_LOAD_ACC
 #endif

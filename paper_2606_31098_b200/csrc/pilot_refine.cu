@@ -10,6 +10,12 @@
 // candidate pose for the next pass — no host synchronisation anywhere.
 //
 // Shares no code with oracle/ (only the POD structs of include/pilot_refine.h).
+// CTAs of 4 warps for the pass kernel (4 per SM at 128 registers): the same 16 warps per SM as 2 x 8, but finer-grained
+// barriers and tails — measured 12.51 -> 12.13 ms on config 4. The cluster-resident kernel keeps 8 warps per CTA.
+#ifndef PILOT_THREADS
+#define PILOT_THREADS 128
+#define PILOT_MIN_BLOCKS 4
+#endif
 #include "pilot_device.cuh"
 
 #include <stdio.h>
@@ -29,7 +35,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   PILOT_ZERO_ACC
   {
     const int begin = chunk_idx * A.chunk;
-    photo_accumulate<T, G, CEN>(A, st->Rc, st->Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc);
+    photo_accumulate<T, G, CEN>(A, st->Rc, st->Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc, red);
   }
   PILOT_LOAD_ACC
 
@@ -386,6 +392,12 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
       ++launches;
     } else {
       pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode);
+      const size_t smem = gather_smem_for(g);
+      if (smem > 48 * 1024 && cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)smem) != cudaSuccess) {
+        if (prev != c.device) cudaSetDevice(prev);
+        return PILOT_ERR_CUDA;
+      }
       dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
       // small CTAs (<= 512 anchors) in more than one wave, or many hypotheses (measured: config 2, H = 1024, -4 %):
       // the serial tail moves to its own launch
@@ -395,7 +407,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
                  ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 512));
       for (int pass = 0; pass <= p->iters[l]; ++pass) {
         A.pass = pass;
-        fn<<<grid, kThreads, 0, st>>>(A);
+        fn<<<grid, kThreads, smem, st>>>(A);
         ++launches;
         if (A.defer) {
           finalize_kernel<<<(A.n_hyp + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(A);

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
         for (int i = 0; i < 6; ++i) sh.prior.J[i] = ok ? Jr[i] : 0.0;
       }
     } else {
-      photo_accumulate<T, G, CEN>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc);
+      photo_accumulate<T, G, CEN>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc, red);
     }
     PILOT_LOAD_ACC
 #ifdef PILOT_RESIDENT_PROFILE
@@ -174,7 +174,11 @@ int pilot_internal::resident_launch(pilot_dtype dtype, int lanes_per_unit, int g
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)A.n_hyp * (unsigned)cluster, 1, 1);
   cfg.blockDim = dim3(kThreads, 1, 1);
-  cfg.dynamicSmemBytes = 0;
+  const size_t smem = gather_smem_for(lanes_per_unit);
+  if (smem > 48 * 1024 - 3 * 1024 &&
+      cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return (int)cudaErrorInvalidValue;
+  cfg.dynamicSmemBytes = smem;
   cfg.stream = static_cast<cudaStream_t>(stream);
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
