@@ -221,7 +221,8 @@ class Streaming:
         L = s.LEVELS
         S = b.Sequence(3, [l[0] for l in L], [l[1] for l in L], [l[2] for l in L], "bf16", s.H, s.N, sum(s.iters),
                        s.offsets, s.dsm, s.origin, s.gsd, s.gravity_world, n + 1)
-        frames = [b.make_frame(f) for f in (self.frames * (n // self.RING + 2))[:n + 1]]
+        ring = [b.make_frame(f, pin=True) for f in self.frames]          # page-locked once; every frame is still uploaded
+        frames = (ring * (n // self.RING + 2))[:n + 1]
         S.set_prior(s.gt_pose(0).reshape(-1), stream)
         S.upload(frames[0]); S.upload(frames[1]); S.step(self.params, stream)      # warm-up frame
         self.torch.cuda.synchronize(self.dev)

@@ -290,6 +290,9 @@ typedef struct {                       /* one frame; HOST pointers, same layouts
   const void*  ref_feat[PILOT_MAX_LEVELS];
   float intrinsics[PILOT_MAX_LEVELS][4];
   float gravity_imu[3], range_ray_cam[3], range_meas;
+  int arrays_pinned;                   /* 1: the arrays above are page-locked (cudaHostAlloc / cudaHostRegister) and stay
+                                          valid and unchanged until this frame's step() has run on the device: they are
+                                          copied straight from the caller's memory (no host staging copy). 0: staged. */
 } pilot_refine_frame;
 
 #define PILOT_SEQ_ROW 16               /* floats per log row: pose[12], cost, best index, n_valid, status */

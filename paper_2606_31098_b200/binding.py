@@ -86,7 +86,8 @@ class Frame(C.Structure):
                 ("query_feat", C.c_void_p * MAX_LEVELS), ("query_conf", C.c_void_p * MAX_LEVELS),
                 ("points", C.c_void_p * MAX_LEVELS), ("ref_feat", C.c_void_p * MAX_LEVELS),
                 ("intrinsics", (C.c_float * 4) * MAX_LEVELS),
-                ("gravity_imu", C.c_float * 3), ("range_ray_cam", C.c_float * 3), ("range_meas", C.c_float)]
+                ("gravity_imu", C.c_float * 3), ("range_ray_cam", C.c_float * 3), ("range_meas", C.c_float),
+                ("arrays_pinned", C.c_int)]
 
 
 DEFAULT_PARAMS = dict(
@@ -460,13 +461,21 @@ def prune_topk(cost, poses, k, stream=None):
 
 # ------------------------------------------------------------------ streaming sequence
 
-def make_frame(prob):
-    """A frame problem dict (host numpy arrays) -> (Frame struct, keep-alive list, bytes uploaded per frame)."""
+def make_frame(prob, pin=False):
+    """A frame problem dict (host numpy arrays) -> (Frame struct, keep-alive list, bytes uploaded per frame).
+    pin=True copies the arrays into page-locked memory once: upload() then DMAs straight from them (they must stay
+    alive and unchanged until the frame was stepped)."""
     f, keep, nbytes = Frame(), [], 0
     L = int(prob["n_levels"])
+    f.arrays_pinned = 1 if pin else 0
     for l in range(L):
         def hold(a, dt=None):
             a = np.ascontiguousarray(a if dt is None else np.asarray(a, dt))
+            if pin and a.size:
+                import torch
+                t = torch.from_numpy(a.view(np.uint8).reshape(-1)).pin_memory()
+                keep.append(t)
+                a = t.numpy().view(a.dtype).reshape(a.shape)
             keep.append(a)
             return a
         q = hold(prob["query_feat"][l])

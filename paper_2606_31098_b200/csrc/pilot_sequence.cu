@@ -180,11 +180,15 @@ int pilot_refine_sequence_upload(pilot_refine_sequence* s, const pilot_refine_fr
   const size_t es = elem_size(c.feat_dtype);
   // the caller's arrays are copied into page-locked staging first (so they may be pageable and reused at once);
   // the previous copy OUT of this staging half (two uploads ago) must have finished before it is overwritten
-  if (S.ready_recorded) ok = ok && cudaEventSynchronize(S.ready) == cudaSuccess;
+  if (S.ready_recorded && !f->arrays_pinned) ok = ok && cudaEventSynchronize(S.ready) == cudaSuccess;
   auto up = [&](size_t at, const void* src, size_t bytes) {
     if (!src || !bytes || !ok) return;
-    memcpy(S.pinned + at, src, bytes);
-    ok = cudaMemcpyAsync(S.base + at, S.pinned + at, bytes, cudaMemcpyHostToDevice, s->copy_stream) == cudaSuccess;
+    if (f->arrays_pinned) {                     // the caller's page-locked arrays are the DMA source
+      ok = cudaMemcpyAsync(S.base + at, src, bytes, cudaMemcpyHostToDevice, s->copy_stream) == cudaSuccess;
+    } else {
+      memcpy(S.pinned + at, src, bytes);
+      ok = cudaMemcpyAsync(S.base + at, S.pinned + at, bytes, cudaMemcpyHostToDevice, s->copy_stream) == cudaSuccess;
+    }
   };
   for (int l = 0; l < c.n_levels; ++l) {
     size_t px = (size_t)c.width[l] * c.height[l], N = (size_t)f->n_points[l];

@@ -115,3 +115,21 @@ def test_sequence_argument_errors():
     # same frame, second step seeded from the first estimate: still at the same optimum
     assert parity.trans_dist(r[0, :12], r[1, :12])[0] < 0.05
     S.close()
+
+
+def test_pinned_frames_are_copied_directly_and_give_the_same_track():
+    from paper_2606_31098_b200 import binding, workloads as wl
+    seq = wl.Config3Sequence(n_frames=6, H=16, N=1024, iters=(2, 2, 2))
+    tracks = []
+    for pin in (False, True):
+        S = make_sequence(seq, 6)
+        S.set_prior(seq.gt_pose(0).reshape(-1))
+        frames = [binding.make_frame(seq.frame(i), pin=pin) for i in range(6)]
+        S.upload(frames[0])
+        for i in range(6):
+            if i + 1 < 6:
+                S.upload(frames[i + 1])
+            S.step(seq.params)
+        tracks.append(S.results())
+        S.close()
+    assert np.array_equal(tracks[0], tracks[1])
