@@ -316,7 +316,12 @@ template <> struct Log2<1> { static constexpr int v = 0; };
 template <int G> struct RedRows {
   static constexpr bool kOn = PILOT_SMEM_RS && G >= 2 && G <= 8;
   static constexpr int kStride = G == 2 ? 12 : (G == 4 ? 28 : (G == 8 ? 52 : 0));
-  static constexpr int kWarpFloats = kOn ? 32 * kStride : 0;
+  // The lane groups that store in the same half-warp phase would hit the same banks (G * kStride is a multiple of 32
+  // words): every group's block of rows is shifted by kSkew more words than the previous one (a multiple of 4, so
+  // rows stay 16-B aligned; cumulative, so rows never overlap).
+  static constexpr int kSkew = G == 8 ? 16 : (G == 4 ? 4 : 0);
+  static constexpr int kWarpFloats = kOn ? 32 * kStride + kSkew * (32 / G) : 0;
+  __device__ static __forceinline__ int row(int u) { return u * kStride + kSkew * (u / G); }
 };
 // dynamic shared memory of the gather kernels: [accumulators kNacc x kThreads] [kWarps reduction buffers]
 inline size_t gather_smem_for(int g);
@@ -427,7 +432,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
         for (int i = 0; i < 6; ++i) cur[i] = 0.f;
       }
       if constexpr (RedRows<G>::kOn) {
-        float2* row = reinterpret_cast<float2*>(red + ((lane & ~(G - 1)) + r) * RedRows<G>::kStride + sub * 6);
+        float2* row = reinterpret_cast<float2*>(red + RedRows<G>::row((lane & ~(G - 1)) + r) + sub * 6);
         row[0] = make_float2(cur[0], cur[1]); row[1] = make_float2(cur[2], cur[3]); row[2] = make_float2(cur[4], cur[5]);
       } else {
 #pragma unroll
@@ -445,7 +450,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
     }
     if constexpr (RedRows<G>::kOn) {                       // lane i sums the G slices of unit i, in lane order
       __syncwarp();
-      const float4* rp = reinterpret_cast<const float4*>(red + lane * RedRows<G>::kStride);
+      const float4* rp = reinterpret_cast<const float4*>(red + RedRows<G>::row(lane));
       float v[6 * G];
 #pragma unroll
       for (int i = 0; i < 6 * G / 4; ++i) {
