@@ -24,8 +24,8 @@ UNIT = "point-hyp-iters/s"
 LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", "iter_cost", "iter_lambda")
 
 # dram__bytes_read.sum + dram__bytes_write.sum per photo_pass_kernel launch from the committed `ncu --set full`
-# capture of this command (profiles/r1_photo_config4.md); None where no capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"config4": 35.0e6}
+# capture of this command (profiles/r1d_photo_config4.md); None where no capture of that workload exists.
+NCU_TRAFFIC_BYTES = {"config4": 35.3e6}
 
 
 def load_peaks():
@@ -487,18 +487,18 @@ def main():
                        "unit": "TFLOP/s", "frac": flops_per_launch / launch_s / 1e12 / alu_peak,
                        "note": "fp32 FMA lanes: 2*(19*C+120) algorithmic flop per unit-evaluation against "
                                "SMs*128*2*1.965 GHz; the kernel is issue/FMA-pipe bound, not byte bound "
-                               "(profiles/r1b_photo_config4.md)"}
+                               "(profiles/r1d_photo_config4.md)"}
     # t_model = max(compulsory HBM bytes / HBM peak, gather bytes / L2 gather peak, flops / FMA
     # peak); the L2 term is filled in below when the probe runs. Instruction issue (warp instructions per unit from
     # the committed ncu captures) is listed beside it because it is the term that binds.
     compulsory = float(map_bytes) / max(1, W.prob["n_levels"])          # one level's map read once per pass
     model = {"t_hbm_compulsory_ms": compulsory / (peak * 1e9) * 1e3, "t_fma_ms": flops_per_launch / (alu_peak * 1e12) * 1e3,
              "t_l2_gather_ms": None, "t_run_ms": launch_s * 1e3}
-    inst_per_unit = {64: 49.0, 32: 32.7}.get(W.prob["channels"][-1]) if W.prob["dtype"] != "f32" else None
+    inst_per_unit = {64: 47.5, 32: 32.7}.get(W.prob["channels"][-1]) if W.prob["dtype"] != "f32" else None
     if inst_per_unit:
         units_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * 2)
         model["t_issue_ms"] = units_per_launch * inst_per_unit / (prop.multi_processor_count * 4 * 1.965e9) * 1e3
-        model["issue_source"] = "warp instructions per unit from profiles/r1b_photo_config4.md (C=64) / r1c (C=32)"
+        model["issue_source"] = "warp instructions per unit from profiles/r1d_photo_config4.md (C=64) / r1c_resident_small_workloads.md (C=32)"
     roofline["model"] = model
     if rank == 0 and not args.no_probe:
         # the build's own micro-benchmark: random gathers with the kernel's access shape
