@@ -103,6 +103,7 @@ class Resident:
         if args.chunk:
             self.ref.set_chunk(args.chunk)
         self.ref.set_exec_mode(args.mode, args.cluster)
+        self.ref.set_math_mode(args.math)
         self.H = prob["init_poses"].shape[0]
         self.units = prob["units"]
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(prob, [self.H] * prob["n_levels"])
@@ -139,6 +140,7 @@ class Resident:
         if self.args.chunk:
             href.set_chunk(self.args.chunk)
         href.set_exec_mode(self.args.mode, self.args.cluster)
+        href.set_math_mode(self.args.math)
         T = sum(self.params["iters"])
         d2h = self.H * (48 + 4 + 4 + 4) + T * self.H * (144 + 24 + 4 + 4)
         href.run(hi, self.params, stream, LIGHT)
@@ -186,6 +188,7 @@ class Streaming:
             di.inp.init_poses_dev = self.seeds.data_ptr()
         self.ref = binding.Refiner.for_inputs(self.di[0], self.params, local_rank)
         self.ref.set_exec_mode(args.mode, args.cluster)
+        self.ref.set_math_mode(args.math)
         self.H, self.units, self.i = seq.H, seq.units_per_frame, 0
         self.prob = dict(self.frames[0], params=self.params)
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(self.prob, [self.H] * 3)
@@ -261,6 +264,7 @@ class PaperSchedule:
         self.di = binding.DeviceInputs(prob, local_rank)
         self.pr = binding.PrunedRefiner(self.di, self.params, self.off, prob["keep"], "world", local_rank)
         self.pr.ref.set_exec_mode(args.mode, args.cluster)
+        self.pr.ref.set_math_mode(args.math)
         self.prior = torch.from_numpy(prob["prior_pose"]).to(torch.device("cuda", local_rank))
         self.H0, self.keep, self.units = self.off.shape[0], prob["keep"], prob["units"]
         self.bytes_per_launch, self.pass_launches = gather_bytes_per_launch(prob, [self.H0, self.keep, self.keep])
@@ -407,6 +411,7 @@ def main():
     ap.add_argument("--config", default="config4", choices=sorted(WORKLOADS))
     ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA of the pass kernel (0 = heuristic)")
     ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident", "split"], help="launch strategy (pilot_exec_mode)")
+    ap.add_argument("--math", default="auto", choices=["auto", "fp32", "mma"], help="per-unit contraction (pilot_math_mode)")
     ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -536,7 +541,7 @@ def main():
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     if rank == 0:
-        cfg = {"workload": args.config, "exec_mode": args.mode}
+        cfg = {"workload": args.config, "exec_mode": args.mode, "math_mode": args.math}
         cfg.update(W.config())
         cfg.update({"map_bytes": map_bytes, "l2_bytes": int(l2_bytes),
                     "l2_policy": "L2 flushed between timed steps" if need_flush else "inputs larger than L2",

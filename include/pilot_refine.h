@@ -192,6 +192,20 @@ int pilot_refine_set_chunk(pilot_refine_handle* h, int chunk);
 typedef enum { PILOT_EXEC_AUTO = 0, PILOT_EXEC_PASSES = 1, PILOT_EXEC_RESIDENT = 2, PILOT_EXEC_PASSES_SPLIT = 3 } pilot_exec_mode;
 int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster);
 
+/*
+ * Arithmetic of the per-unit contraction (Eq.(1),(8) PAPER.md:118,160-164). FP32: taps are
+ * unpacked to fp32 and every step runs on the FMA pipe (packed FFMA2). MMA: for 16-bit features (bf16 / fp16) with
+ * 16, 32, 64 or 128 channels and the exact bilinear gradient, the first differences of the taps are taken in the
+ * storage type (exact for neighbouring values within a factor of two; else one rounding of 2^-9 / 2^-12 relative to
+ * the difference), and their 4 x 4 Gram matrix per unit is accumulated in fp32 on the tensor cores (mma.sync
+ * m16n8k16); the bilinear combination follows in fp32. AUTO (default) = MMA where it applies AND was measured faster
+ * (64 or more channels on the one-launch-per-pass strategy), FP32 elsewhere. Asking for MMA where it does not apply
+ * falls back to FP32 (not an error). Results agree within the bf16 / fp16 parity
+ * tolerance of the path (5e-3 relative on H and g); fp32 features always use FP32.
+ */
+typedef enum { PILOT_MATH_AUTO = 0, PILOT_MATH_FP32 = 1, PILOT_MATH_MMA = 2 } pilot_math_mode;
+int pilot_refine_set_math_mode(pilot_refine_handle* h, int mode);
+
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */
 int pilot_refine_last_launches(const pilot_refine_handle* h);
 

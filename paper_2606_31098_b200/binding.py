@@ -22,12 +22,13 @@ ERRORS = {-1: "bad argument", -2: "workspace too small", -3: "unsupported shape 
 
 SEED_CODE = {"camera": 0, "world": 1}
 EXEC_CODE = {"auto": 0, "passes": 1, "resident": 2, "split": 3}
+MATH_CODE = {"auto": 0, "fp32": 1, "mma": 2}
 TOPK_MAX = 8192
 
 EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_run", "pilot_refine_destroy",
            "pilot_refine_create_host", "pilot_refine_run_host", "pilot_refine_submit_host",
            "pilot_refine_wait_host", "pilot_refine_last_launches",
-           "pilot_refine_run_levels", "pilot_refine_set_exec_mode", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
+           "pilot_refine_run_levels", "pilot_refine_set_exec_mode", "pilot_refine_set_math_mode", "pilot_refine_grid_offsets", "pilot_refine_seed_hypotheses",
            "pilot_refine_select_best", "pilot_refine_prune_topk",
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
@@ -128,6 +129,8 @@ def lib():
         L.pilot_refine_set_chunk.restype = C.c_int
         L.pilot_refine_set_exec_mode.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.pilot_refine_set_exec_mode.restype = C.c_int
+        L.pilot_refine_set_math_mode.argtypes = [C.c_void_p, C.c_int]
+        L.pilot_refine_set_math_mode.restype = C.c_int
         L.pilot_refine_run_levels.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.POINTER(Outputs),
                                               C.c_int, C.c_int, C.c_void_p]
         L.pilot_refine_run_levels.restype = C.c_int
@@ -329,6 +332,9 @@ class Refiner:
     def set_exec_mode(self, mode="auto", cluster=0):
         _check(lib().pilot_refine_set_exec_mode(self.handle, EXEC_CODE[mode], int(cluster)), "pilot_refine_set_exec_mode")
 
+    def set_math_mode(self, math="auto"):
+        _check(lib().pilot_refine_set_math_mode(self.handle, MATH_CODE[math]), "pilot_refine_set_math_mode")
+
     def set_chunk(self, chunk):
         _check(lib().pilot_refine_set_chunk(self.handle, int(chunk)), "pilot_refine_set_chunk")
 
@@ -379,13 +385,14 @@ class Refiner:
             pass
 
 
-def refine(prob, params=None, device=0, mode="auto", cluster=0):
+def refine(prob, params=None, device=0, mode="auto", cluster=0, math="auto"):
     """One-shot convenience: upload a problem dict, run, synchronise, return numpy outputs."""
     torch = _torch()
     di = DeviceInputs(prob, device)
     P = dict(prob.get("params", {})); P.update(params or {})
     r = Refiner.for_inputs(di, P, device)
     r.set_exec_mode(mode, cluster)
+    r.set_math_mode(math)
     out = r.run(di, P)
     torch.cuda.synchronize(device)
     res = {k: v.cpu().numpy() for k, v in out.items()}

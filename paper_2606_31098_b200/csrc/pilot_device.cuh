@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace {
 
@@ -89,7 +90,7 @@ struct PassArgs {
 
 // pilot_resident.cu: one launch of the cluster-resident LM kernel for the level described by A (A.lv, A.level,
 // A.iters, A.rec_base): `cluster` CTAs per hypothesis. Returns a cudaError_t as int.
-int resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, const PassArgs& A, int cluster, void* stream);
+int resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, bool mma, const PassArgs& A, int cluster, void* stream);
 
 }  // namespace pilot_internal
 using namespace pilot_internal;
@@ -323,10 +324,345 @@ template <int G> struct RedRows {
   static constexpr int kWarpFloats = kOn ? 32 * kStride + kSkew * (32 / G) : 0;
   __device__ static __forceinline__ int row(int u) { return u * kStride + kSkew * (u / G); }
 };
+// ------------------------------------------------------------------ tensor-core variant of the per-unit contraction
+//
+// For 16-bit features the C x 3 contraction of a unit (a3-a5) is a 4 x 4 Gram matrix E = D D^T of FIRST DIFFERENCES
+//   e0 = f10 - f00,  e1 = f11 - f01,  e2 = f01 - f00,  e3 = ref - f01          (rows of D, C channels each)
+// followed by three quadratic forms in the bilinear weights (mma_unit_scalars below):
+//   gx = (1-b) e0 + b e1,   gy = -a e0 + a e1 + e2,   r = f - ref = a(1-b) e0 + ab e1 + (b-1) e2 - e3.
+// The differences are taken in the storage type (packed HSUB2: exact whenever the two values are within a factor of two
+// of each other - Sterbenz - which is every channel of a smooth map except at zero crossings; otherwise one rounding of
+// 2^-9 (bf16) / 2^-12 (fp16) relative to the DIFFERENCE, not to the taps), their products are exact and accumulate in
+// fp32 on the tensor cores (mma.sync.m16n8k16 = HMMA.16816.F32). Differencing first is what makes the Gram safe: a
+// Gram of the raw taps would cancel by ~3e4.
+//
+// One mma covers 16 rows = (units of the round) x (32-channel slices of a pixel) x {e0, e1 | e2, e3}: thread (g, q) of
+// the fragment layout (g = lane / 4, q = lane % 4) supplies rows g and g + 8 for the channels of its 16-byte load, so
+// g = (unit, sel, slice): sel 0 loads f00, f10, f01 -> rows e0 | e2; sel 1 loads f01, f11, ref -> rows e1 | e3. The four
+// q-threads x two slices of a pixel read one full 128-byte line per load instruction (C = 64), as the fp32 path does.
+// B is the same registers (the Gram is symmetric): mma #1 multiplies by rows 0-7 (e0, e1), mma #2 by rows 8-15 (e2, e3);
+// only the 4 x 4 diagonal blocks (same unit, same slice) are used.
+template <class T> struct MmaType;
+template <> struct MmaType<BF16Tag> {
+  static __device__ __forceinline__ unsigned sub2(unsigned x, unsigned y) {
+    unsigned d;
+    asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(d) : "r"(x), "r"(y));
+    return d;
+  }
+  static __device__ __forceinline__ void mma(float (&c)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+  }
+};
+template <> struct MmaType<F16Tag> {
+  static __device__ __forceinline__ unsigned sub2(unsigned x, unsigned y) {
+    unsigned d;
+    asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(x), "r"(y));
+    return d;
+  }
+  static __device__ __forceinline__ void mma(float (&c)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+  }
+};
+template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features stay on the FFMA2 path
+
+#ifndef PILOT_MMA_XBATCH
+#define PILOT_MMA_XBATCH 1      // 1: anchors and projection of the NEXT batch overlap the first taps of the current one
+                                // (config 4, prefetch 6: 12.57 ms without, 11.27 ms with)
+#endif
+#ifndef PILOT_MMA_SHFL_ACC
+#define PILOT_MMA_SHFL_ACC 0
+#endif
+#ifndef PILOT_MMA_PREFETCH
+#define PILOT_MMA_PREFETCH 6    // rounds whose taps are in flight ahead of the tensor-core arithmetic
+#endif
+
+template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
+  static constexpr int KS = CH >= 32 ? 2 : 1;          // k-steps of 16 channels per mma chain
+  static constexpr int KH = CH >= 32 ? CH / 32 : 1;    // 32-channel slices per pixel
+  static constexpr int LOGKH = KH == 4 ? 2 : (KH == 2 ? 1 : 0);
+  static constexpr int NW = 2 * KS;                    // 32-bit words (= pairs of channels) per load per thread
+  static constexpr int LB = 4 * NW;                    // bytes per load per thread
+  static constexpr int UR = 4 / KH;                    // units per round
+  static constexpr int ROUNDS = 32 / UR;
+  static constexpr int PX = CH * 2;                    // bytes per pixel
+  static constexpr int kStride = 16 * KH + 4;          // floats per unit row of the warp's buffer: [KH][4][4] + pad (odd
+                                                       // multiple of 4 words: the lanes' LDS.128 are conflict-free)
+  static constexpr int kWarpFloats = 32 * kStride;
+};
+template <int G> __host__ __device__ constexpr bool mma_supported() { return G == 2 || G == 4 || G == 8 || G == 16; }
+
+template <int NW> struct TapWords { unsigned w[NW]; };
+template <int NW> __device__ __forceinline__ TapWords<NW> ldg_words(const char* p) {
+  TapWords<NW> t;
+  if constexpr (NW == 4) {
+    const uint4 v = ldg16(p);
+    t.w[0] = v.x; t.w[1] = v.y; t.w[2] = v.z; t.w[3] = v.w;
+  } else {
+    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p));
+    t.w[0] = v.x; t.w[1] = v.y;
+  }
+  return t;
+}
+
+// Lane phase: lane i reads the Gram matrix of unit i (summing the 32-channel slices in a fixed order) and forms
+//   p = { gx.gx, gx.gy, gy.gy, gx.r, gy.r, r.r } = M E M^T, M = rows of the three combinations above.
+template <int CH>
+__device__ __forceinline__ void mma_unit_scalars(const float* red, int lane, float a, float b, float (&p)[6]) {
+  using Geo = MmaGeom<CH>;
+  const float4* rp = reinterpret_cast<const float4*>(red + lane * Geo::kStride);
+  float F[16], E[16];                                                     // F: the order the fragments were stored in
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { const float4 t = rp[i]; F[4 * i] = t.x; F[4 * i + 1] = t.y; F[4 * i + 2] = t.z; F[4 * i + 3] = t.w; }
+#pragma unroll
+  for (int k = 1; k < Geo::KH; ++k) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const float4 t = rp[4 * k + i]; F[4 * i] += t.x; F[4 * i + 1] += t.y; F[4 * i + 2] += t.z; F[4 * i + 3] += t.w; }
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      E[4 * i + j] = Geo::KH == 1 ? F[(i & 1) * 8 + (j >> 1) * 4 + (i >> 1) * 2 + (j & 1)]
+                                  : F[(i & 1) * 8 + (j & 1) * 4 + (j >> 1) * 2 + (i >> 1)];
+  const float ob = 1.f - b, m20 = a * ob, m21 = a * b, m22 = b - 1.f;
+  float t0[2], t1[3], t2[4];                                              // t_k = E m_k (the rows that are needed)
+#pragma unroll
+  for (int i = 0; i < 2; ++i) t0[i] = ob * E[4 * i] + b * E[4 * i + 1];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) t1[i] = a * (E[4 * i + 1] - E[4 * i]) + E[4 * i + 2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) t2[i] = m20 * E[4 * i] + m21 * E[4 * i + 1] + m22 * E[4 * i + 2] - E[4 * i + 3];
+  p[0] = ob * t0[0] + b * t0[1];
+  p[1] = ob * t1[0] + b * t1[1];
+  p[2] = a * (t1[1] - t1[0]) + t1[2];
+  p[3] = ob * t2[0] + b * t2[1];
+  p[4] = a * (t2[1] - t2[0]) + t2[2];
+  p[5] = m20 * t2[0] + m21 * t2[1] + m22 * t2[2] - t2[3];
+}
+
+// floats of the [kNacc][kThreads] accumulator array in dynamic shared memory (0: accumulators in registers)
+template <bool MMA> __host__ __device__ constexpr int acc_smem_floats() {
+  return (MMA && PILOT_MMA_SHFL_ACC) ? 0 : (PILOT_SMEM_ACC ? kNacc * kThreads : 0);
+}
+template <int G, bool MMA> __host__ __device__ constexpr int red_warp_floats() {
+  if constexpr (MMA) return MmaGeom<8 * G>::kWarpFloats; else return RedRows<G>::kWarpFloats;
+}
+
 // dynamic shared memory of the gather kernels: [accumulators kNacc x kThreads] [kWarps reduction buffers]
-inline size_t gather_smem_for(int g);
-template <int G> constexpr size_t gather_smem_bytes() {
-  return (size_t)(PILOT_SMEM_ACC ? kNacc * kThreads : 0) * 4 + (size_t)kWarps * RedRows<G>::kWarpFloats * 4;
+inline size_t gather_smem_for(int g, bool mma);
+template <int G, bool MMA> constexpr size_t gather_smem_bytes() {
+  return (size_t)acc_smem_floats<MMA>() * 4 + (size_t)kWarps * red_warp_floats<G, MMA>() * 4;
+}
+
+// ------------------------------------------------------------------ the photo gather, tensor-core contraction
+//
+// Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on batches of 32 units:
+//   lane-per-unit   anchor load, projection + visibility in fp64 (a2) - done ONE BATCH AHEAD, while the first taps
+//                   of the current batch are in flight, so that the tap latency at the head of a batch is covered;
+//   fragment roles  ROUNDS rounds of (HSUB2 differences -> 2 KS mma.sync) over UR units each, taps prefetched
+//                   PILOT_MMA_PREFETCH rounds ahead; the 4 x 4 diagonal blocks go to the warp's buffer `red`;
+//   lane-per-unit   Gram -> six scalars, robust weight, lift through J_uv, accumulate (a4-a6).
+template <class T, int G>
+__device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const double* Rc, const double* Ccand,
+                                                     int begin, int end, int worker, int n_workers,
+                                                     float (&acc)[kNacc], float* sacc, float* red) {
+#if PILOT_SMEM_ACC
+#define PILOT_MACC(i) sacc[(i) * kThreads]
+#else
+#define PILOT_MACC(i) acc[i]
+#endif
+  constexpr int CH = 8 * G;
+  using Geo = MmaGeom<CH>;
+  using M = MmaType<T>;
+  constexpr int NW = Geo::NW, PX = Geo::PX, ROUNDS = Geo::ROUNDS;
+  constexpr int PF = PILOT_MMA_PREFETCH < ROUNDS ? PILOT_MMA_PREFETCH : ROUNDS;
+  const LevelArgs& L = A.lv;
+  const int lane = threadIdx.x & 31;
+  const unsigned row_stride = (unsigned)PX * (unsigned)L.W;
+  const char* feat = static_cast<const char*>(L.feat);
+  const char* refb = static_cast<const char*>(L.ref);
+
+  // The candidate pose stays in SHARED memory (Rc, Ccand must point there) and is re-read by every projection: as 24
+  // registers held across the rounds it forced the address arithmetic of every round to be rematerialised.
+  const volatile double* R = Rc;
+  const volatile double* Cc = Ccand;
+  const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
+
+  // fragment roles: g = (uu, sel, slice), slice in the low bits: the 8 lanes of a quarter-warp (one phase of a 16-byte
+  // load) cover one contiguous 128-byte line (C >= 64) - with sel below the slice every phase touches two lines
+  // (measured: 15.5 ms instead of 12.7 on config 4). Round r works on the units u0 + r (the owner's lane is an
+  // immediate of the shuffle).
+  const int q = lane & 3, g = lane >> 2;
+  const int kap = g & (Geo::KH - 1), sel = (g >> Geo::LOGKH) & 1, uu = g >> (1 + Geo::LOGKH);
+  const int u0 = uu * ROUNDS;
+  const unsigned tofs = (unsigned)(kap * 64 + q * Geo::LB);
+  const char* pA = feat + tofs + (sel ? row_stride : 0u);                 // + offset: f00 | f01;  + PX: f10 | f11
+  const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
+  float* const srow = red + u0 * Geo::kStride + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
+  bool useful; int js = 0;
+  if constexpr (Geo::KH == 1) useful = q == uu;
+  else { useful = Geo::KH == 2 ? (q >> 1) == uu : (q & 1) == (kap >> 1); js = Geo::KH == 2 ? (q & 1) : (q >> 1); }
+  const bool odd = kap & 1;
+
+  struct Unit { float a, b, X, Y, iz, w; unsigned off; bool valid; };
+  auto load_anchor = [&](int base) { const int j = base + lane; return j < end ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
+  auto project = [&](const float4& P, int base) {                         // a2, in double so that u, v carry no fp32 noise
+    Unit U;
+    bool valid = base + lane < end;
+    double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
+    double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
+    double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
+    double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
+    valid = valid && (Zd > (double)A.prm.z_near);
+    double izd = fast_rcp(Zd);
+    double ud = (double)L.fx * Xd * izd + (double)L.cx;
+    double vd = (double)L.fy * Yd * izd + (double)L.cy;
+    double x0d = floor(ud), y0d = floor(vd);
+    valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
+    U.a = valid ? (float)(ud - x0d) : 0.f;
+    U.b = valid ? (float)(vd - y0d) : 0.f;
+    const int x0 = valid ? (int)x0d : 0, y0 = valid ? (int)y0d : 0;
+    U.off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * (unsigned)PX;   // invisible units gather pixel (0,0)
+    U.X = (float)Xd; U.Y = (float)Yd; U.iz = (float)izd; U.w = P.w; U.valid = valid;
+    return U;
+  };
+
+  struct Raw { TapWords<NW> l0, l1, l2; };
+  const int step = n_workers * 32;
+  int base = begin + worker * 32;
+  if (base >= end) return;
+#if PILOT_MMA_XBATCH
+  float4 Pn = load_anchor(base);
+  Unit cur = project(Pn, base);
+  Pn = load_anchor(base + step);
+#endif
+  for (; base < end; base += step) {
+#if !PILOT_MMA_XBATCH
+    const Unit cur = project(load_anchor(base), base);
+#endif
+    // the batch's reference rows are contiguous; a batch that runs over the end of the anchors clamps its rows
+    const char* const p2 = sel ? refb + (size_t)base * PX + tofs : pF;     // + offset: ref | f01
+    const unsigned jmaxPX = (unsigned)min(31, L.N - 1 - base) * (unsigned)PX;
+    const unsigned u0PX = (unsigned)(u0 * PX);
+    auto fetch = [&](int r) {
+      const unsigned o = __shfl_sync(0xffffffffu, cur.off, r, ROUNDS);    // lane u0 + r
+      const unsigned o2 = sel ? min(u0PX + (unsigned)(r * PX), jmaxPX) : o;
+      Raw t;
+      t.l0 = ldg_words<NW>(pA + o);
+      t.l1 = ldg_words<NW>(pA + o + PX);
+      t.l2 = ldg_words<NW>(p2 + o2);
+      return t;
+    };
+    Raw buf[PF];
+#pragma unroll
+    for (int d = 0; d < PF; ++d) buf[d] = fetch(d);
+
+#if PILOT_MMA_XBATCH
+    // next batch: projection while the first taps are in flight; its anchors were loaded one batch ago
+    const Unit nxt = project(Pn, base + step);
+    Pn = load_anchor(base + 2 * step);
+#endif
+
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) {
+      const Raw t = buf[r % PF];
+      if (r + PF < ROUNDS) buf[r % PF] = fetch(r + PF);
+      unsigned eA[NW], eB[NW];
+#pragma unroll
+      for (int i = 0; i < NW; ++i) { eA[i] = M::sub2(t.l1.w[i], t.l0.w[i]); eB[i] = M::sub2(t.l2.w[i], t.l0.w[i]); }
+      float c1[4] = {0.f, 0.f, 0.f, 0.f}, c2[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int s = 0; s < Geo::KS; ++s) {
+        M::mma(c1, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eA[2 * s], eA[2 * s + 1]);
+        M::mma(c2, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eB[2 * s], eB[2 * s + 1]);
+      }
+      // The 4 x 4 diagonal blocks. Column n = 2q + c of the fragments is row-group n = (uu', sel', slice').
+      float4* row = reinterpret_cast<float4*>(srow + r * Geo::kStride);
+      if constexpr (Geo::KH == 1) {                                       // n = (uu' = q, sel' = c): one thread has both columns
+        if (useful) {    // c1 = E[sel][0], E[sel][1], E[2+sel][0], E[2+sel][1];  c2 = the same rows, columns 2 and 3
+          row[0] = make_float4(c1[0], c1[1], c1[2], c1[3]);
+          row[1] = make_float4(c2[0], c2[1], c2[2], c2[3]);
+        }
+      } else {                                                            // slice' = c (KH 2) or 2 (q & 1) + c (KH 4)
+        if (useful)      // E[sel][js], E[2+sel][js], E[sel][2+js], E[2+sel][2+js]
+          row[js] = make_float4(odd ? c1[1] : c1[0], odd ? c1[3] : c1[2], odd ? c2[1] : c2[0], odd ? c2[3] : c2[2]);
+      }
+    }
+    __syncwarp();
+    float p[6];
+    mma_unit_scalars<CH>(red, lane, cur.a, cur.b, p);
+    __syncwarp();                                                         // rows are rewritten by the next batch
+
+    // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
+#if PILOT_MMA_SHFL_ACC
+    float v[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = 0.f;
+#endif
+    if (cur.valid) {
+      const float a = cur.a, b = cur.b;
+      float wq = 1.f;
+      if (L.conf) {
+        const float* cq = L.conf + cur.off / (unsigned)PX;
+        float q00 = __ldg(cq), q10 = __ldg(cq + 1), q01 = __ldg(cq + L.W), q11 = __ldg(cq + L.W + 1);
+        wq = (1.f - b) * ((1.f - a) * q00 + a * q10) + b * ((1.f - a) * q01 + a * q11);
+      }
+      float w = cur.w * wq;
+      float rho, drho;
+      robust<float>(A.prm.loss, w * p[5], A.prm.loss_scale, rho, drho);
+      float om = w * drho;
+      float x = cur.X * cur.iz, y = cur.Y * cur.iz;
+      float fxz = L.fx * cur.iz, fyz = L.fy * cur.iz;
+      float Ju[6] = {fxz, 0.f, -fxz * x, -L.fx * x * y, L.fx * (1.f + x * x), -L.fx * y};
+      float Jv[6] = {0.f, fyz, -fyz * y, -L.fy * (1.f + y * y), L.fy * x * y, L.fy * x};
+      float A11 = om * p[0], A12 = om * p[1], A22 = om * p[2];
+      float b1 = om * p[3], b2 = om * p[4];
+#if PILOT_MMA_SHFL_ACC
+#pragma unroll
+      for (int i = 0; i < 6; ++i) {
+        float mu = A11 * Ju[i] + A12 * Jv[i];
+        float mv = A12 * Ju[i] + A22 * Jv[i];
+#pragma unroll
+        for (int k = i; k < 6; ++k) v[tri(i, k)] = mu * Ju[k] + mv * Jv[k];
+        v[21 + i] = b1 * Ju[i] + b2 * Jv[i];
+      }
+      v[27] = rho;
+      v[28] = 1.f;
+#else
+#pragma unroll
+      for (int i = 0; i < 6; ++i) {
+        float mu = A11 * Ju[i] + A12 * Jv[i];
+        float mv = A12 * Ju[i] + A22 * Jv[i];
+#pragma unroll
+        for (int k = i; k < 6; ++k) PILOT_MACC(tri(i, k)) += mu * Ju[k] + mv * Jv[k];
+        PILOT_MACC(21 + i) += b1 * Ju[i] + b2 * Jv[i];
+      }
+      PILOT_MACC(27) += rho;
+      PILOT_MACC(28) += 1.f;
+#endif
+    }
+#if PILOT_MMA_SHFL_ACC
+    // reduce-scatter of the batch over the warp: lane i ends with the batch total of component i (31 shuffles), which
+    // goes to ONE accumulator register per lane: no shared-memory traffic, no 29 live registers
+#pragma unroll
+    for (int half = 16; half >= 1; half >>= 1) {
+      const bool upper = lane & half;
+#pragma unroll
+      for (int i = 0; i < half; ++i) {
+        const float send = upper ? v[i] : v[i + half];
+        const float keep = upper ? v[i + half] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+      }
+    }
+    acc[0] += v[0];
+#endif
+#if PILOT_MMA_XBATCH
+    cur = nxt;
+#endif
+  }
+#undef PILOT_MACC
 }
 
 // ------------------------------------------------------------------ the photo kernel
@@ -334,7 +670,7 @@ template <int G> constexpr size_t gather_smem_bytes() {
 // grid = (n_hyp, n_chunks): blockIdx.x (fastest) is the hypothesis, so CTAs that run together
 // sweep the SAME chunk of (spatially sorted) anchors under different poses and the union of their
 // footprints is a narrow band of the map that stays in L2.
-template <class T, int G, bool CEN>
+template <class T, int G, bool CEN, bool MMA>
 __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double* Rc, const double* Ccand,
                                                  int begin, int end, int worker, int n_workers,
                                                  float (&acc)[kNacc], float* sacc, float* red /* this warp's rows */) {
@@ -343,6 +679,11 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
 #else
 #define PILOT_ACC(i) acc[i]
 #endif
+  if constexpr (MMA) {
+    static_assert(!CEN && mma_supported<G>() && T::kVec == 8, "tensor-core path: 16-bit features, exact bilinear gradient");
+    photo_accumulate_mma<T, G>(A, Rc, Ccand, begin, end, worker, n_workers, acc, sacc, red);
+    return;
+  }
   constexpr int LOG = Log2<G>::v;
   const LevelArgs& L = A.lv;
   const int lane = threadIdx.x & 31;
@@ -385,8 +726,8 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
 
     // ---- group rounds: gather + per-unit contraction (a3-a5), reduce-scatter so that lane i ends
     //      up with the six sums of unit i of this batch
-    float stash[LOG > 0 ? LOG : 1][6];
     float cur[6];
+    float stash[LOG > 0 ? LOG : 1][6];
     const int gbase = base + (lane & ~(G - 1));           // first unit of this lane's group
     auto fetch = [&](int r, float& ra, float& rb, bool& rvalid) {
       unsigned o = __shfl_sync(0xffffffffu, offv, r, G);
@@ -502,31 +843,54 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
 #undef PILOT_ACC
 }
 
-inline size_t gather_smem_for(int g) {
+inline size_t gather_smem_for(int g, bool mma) {
   switch (g) {
-    case 1: return gather_smem_bytes<1>();
-    case 2: return gather_smem_bytes<2>();
-    case 4: return gather_smem_bytes<4>();
-    case 8: return gather_smem_bytes<8>();
-    case 16: return gather_smem_bytes<16>();
-    case 32: return gather_smem_bytes<32>();
+    case 1: return gather_smem_bytes<1, false>();
+    case 2: return mma ? gather_smem_bytes<2, true>() : gather_smem_bytes<2, false>();
+    case 4: return mma ? gather_smem_bytes<4, true>() : gather_smem_bytes<4, false>();
+    case 8: return mma ? gather_smem_bytes<8, true>() : gather_smem_bytes<8, false>();
+    case 16: return mma ? gather_smem_bytes<16, true>() : gather_smem_bytes<16, false>();
+    case 32: return gather_smem_bytes<32, false>();
   }
   return 0;
 }
 
-// The per-thread accumulators before / after photo_accumulate (registers, or a column of shared memory).
-#if PILOT_SMEM_ACC
+// The per-thread accumulators before / after photo_accumulate: registers, a column of shared memory, or (tensor-core
+// path with PILOT_MMA_SHFL_ACC) one register per lane that already holds the warp total of component `lane`.
 #define PILOT_DECLARE_ACC extern __shared__ float4 pilot_dyn_smem[]; \
   float* sacc = reinterpret_cast<float*>(pilot_dyn_smem) + threadIdx.x; float acc[kNacc]; \
-  float* red = reinterpret_cast<float*>(pilot_dyn_smem) + kNacc * kThreads + (threadIdx.x >> 5) * RedRows<G>::kWarpFloats;
-#define PILOT_ZERO_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) sacc[i * kThreads] = 0.f;
-#define PILOT_LOAD_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) acc[i] = sacc[i * kThreads];
-#else
-#define PILOT_DECLARE_ACC extern __shared__ float4 pilot_dyn_smem[]; float* sacc = nullptr; float acc[kNacc]; \
-  float* red = reinterpret_cast<float*>(pilot_dyn_smem) + (threadIdx.x >> 5) * RedRows<G>::kWarpFloats;
-#define PILOT_ZERO_ACC  _Pragma("unroll") for (int i = 0; i < kNacc; ++i) acc[i] = 0.f;
-#define PILOT_LOAD_ACC
-#endif
+  float* red = reinterpret_cast<float*>(pilot_dyn_smem) + acc_smem_floats<MMA>() + (threadIdx.x >> 5) * red_warp_floats<G, MMA>();
+
+template <bool MMA>
+__device__ __forceinline__ void acc_zero(float (&acc)[kNacc], float* sacc) {
+  if constexpr (MMA && PILOT_MMA_SHFL_ACC) { acc[0] = 0.f; return; }
+#pragma unroll
+  for (int i = 0; i < kNacc; ++i) {
+    if (PILOT_SMEM_ACC) sacc[i * kThreads] = 0.f; else acc[i] = 0.f;
+  }
+}
+
+// Warp total of component `lane` (fixed order: deterministic).
+template <bool MMA>
+__device__ __forceinline__ float acc_warp_total(float (&acc)[kNacc], const float* sacc, int lane) {
+  if constexpr (MMA && PILOT_MMA_SHFL_ACC) return acc[0];
+  if (PILOT_SMEM_ACC) {
+#pragma unroll
+    for (int i = 0; i < kNacc; ++i) acc[i] = sacc[i * kThreads];
+  }
+  // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
+#pragma unroll
+  for (int half = 16; half >= 1; half >>= 1) {
+    const bool upper = lane & half;
+#pragma unroll
+    for (int i = 0; i < half; ++i) {
+      float send = upper ? acc[i] : acc[i + half];
+      float keep = upper ? acc[i + half] : acc[i];
+      acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+    }
+  }
+  return acc[0];
+}
 
 }  // namespace
 

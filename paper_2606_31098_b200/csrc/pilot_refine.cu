@@ -25,36 +25,32 @@ namespace {
 
 // ------------------------------------------------------------------ kernels
 
-template <class T, int G, bool CEN>
+template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
   const int m = blockIdx.x, chunk_idx = blockIdx.y;
   const HypState* st = A.state + m;
   if (st->level != A.level) return;             // finished this level early (failed factorisations)
 
   PILOT_DECLARE_ACC
-  PILOT_ZERO_ACC
+  acc_zero<MMA>(acc, sacc);
   {
     const int begin = chunk_idx * A.chunk;
-    photo_accumulate<T, G, CEN>(A, st->Rc, st->Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc, red);
-  }
-  PILOT_LOAD_ACC
-
-  // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int half = 16; half >= 1; half >>= 1) {
-    const bool upper = lane & half;
-#pragma unroll
-    for (int i = 0; i < half; ++i) {
-      float send = upper ? acc[i] : acc[i + half];
-      float keep = upper ? acc[i + half] : acc[i];
-      acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+    const double* Rc = st->Rc;
+    const double* Cc = st->Cc;
+    if constexpr (MMA) {                          // the tensor-core gather re-reads the pose from shared memory
+      __shared__ double s_pose[12];
+      if (threadIdx.x < 12) s_pose[threadIdx.x] = threadIdx.x < 9 ? st->Rc[threadIdx.x] : st->Cc[threadIdx.x - 9];
+      __syncthreads();
+      Rc = s_pose; Cc = s_pose + 9;
     }
+    photo_accumulate<T, G, CEN, MMA>(A, Rc, Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc, red);
   }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
   __shared__ float s_part[kWarps][kNacc];
   __shared__ float s_sum[kNacc];
   __shared__ int s_last;
-  s_part[warp][lane] = acc[0];
+  s_part[warp][lane] = wtot;
   __syncthreads();
   if (warp == 0) {
     float t = 0.f;
@@ -131,6 +127,7 @@ struct pilot_refine_handle {
   int chunk_override;       // 0 = heuristic
   int mode;                 // pilot_exec_mode
   int cluster_override;     // 0 = heuristic
+  int math_mode;            // pilot_math_mode
   int sm_count;
   int last_launches;
   // host-path staging (create_host only)
@@ -184,12 +181,35 @@ typedef void (*pass_fn)(const PassArgs);
 template <class T, bool CEN>
 pass_fn pick_g(int g) {
   switch (g) {
-    case 1: return photo_pass_kernel<T, 1, CEN>;
-    case 2: return photo_pass_kernel<T, 2, CEN>;
-    case 4: return photo_pass_kernel<T, 4, CEN>;
-    case 8: return photo_pass_kernel<T, 8, CEN>;
-    case 16: return photo_pass_kernel<T, 16, CEN>;
-    case 32: return photo_pass_kernel<T, 32, CEN>;
+#ifndef PILOT_FAST_BUILD
+    case 1: return photo_pass_kernel<T, 1, CEN, false>;
+#endif
+#ifndef PILOT_FAST_BUILD
+    case 2: return photo_pass_kernel<T, 2, CEN, false>;
+#endif
+    case 4: return photo_pass_kernel<T, 4, CEN, false>;
+    case 8: return photo_pass_kernel<T, 8, CEN, false>;
+#ifndef PILOT_FAST_BUILD
+    case 16: return photo_pass_kernel<T, 16, CEN, false>;
+#endif
+#ifndef PILOT_FAST_BUILD
+    case 32: return photo_pass_kernel<T, 32, CEN, false>;
+#endif
+  }
+  return nullptr;
+}
+
+template <class T>
+pass_fn pick_mma(int g) {
+  switch (g) {
+#ifndef PILOT_FAST_BUILD
+    case 2: return photo_pass_kernel<T, 2, false, true>;
+#endif
+    case 4: return photo_pass_kernel<T, 4, false, true>;
+    case 8: return photo_pass_kernel<T, 8, false, true>;
+#ifndef PILOT_FAST_BUILD
+    case 16: return photo_pass_kernel<T, 16, false, true>;
+#endif
   }
   return nullptr;
 }
@@ -197,16 +217,22 @@ pass_fn pick_g(int g) {
 template <bool CEN>
 pass_fn pick_t(pilot_dtype d, int g) {
   switch (d) {
+#ifndef PILOT_FAST_BUILD      /* tuning builds (-DPILOT_FAST_BUILD): bf16, 32 and 64 channels only */
     case PILOT_F32: return pick_g<F32Tag, CEN>(g);
-    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
     case PILOT_F16: return pick_g<F16Tag, CEN>(g);
+#endif
+    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
   }
   return nullptr;
 }
 
-pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode) {
+pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode, bool mma) {
+  if (mma) return d == PILOT_BF16 ? pick_mma<BF16Tag>(g) : pick_mma<F16Tag>(g);
   return grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(d, g) : pick_t<false>(d, g);
 }
+
+// Tensor-core contraction (pilot_math_mode): 16-bit features, 16-128 channels, exact bilinear gradient.
+bool use_mma(const pilot_refine_handle* h, int g, int grad_mode, bool resident);
 
 // Small problems (few (anchor, hypothesis) units per level) are launch- and tail-latency bound with one launch per
 // pass: they go to the cluster-resident kernel, one launch per level. Returns the cluster size, 0 = pass kernel.
@@ -219,6 +245,15 @@ int choose_resident(const pilot_refine_handle* h, int n_hyp, int n_points) {
   int s = 8;
   while (s > 1 && ((long)n_hyp * s > 2L * h->sm_count || n_points / s < 200)) s >>= 1;
   return s;
+}
+
+bool use_mma(const pilot_refine_handle* h, int g, int grad_mode, bool resident) {
+  if (h->math_mode == PILOT_MATH_FP32) return false;
+  const bool applies = h->cfg.feat_dtype != PILOT_F32 && grad_mode == PILOT_GRAD_BILINEAR_EXACT && (g == 2 || g == 4 || g == 8 || g == 16);
+  if (h->math_mode == PILOT_MATH_MMA) return applies;
+  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.93 -> 11.27, config 2 11.46 -> 10.90 (64 channels, one
+  // launch per pass); config 1 0.67 -> 0.75, config 3 1.12 -> 1.24, paper schedule 0.32 -> 0.34 (32 channels, cluster-resident)
+  return applies && g >= 8 && !resident;
 }
 
 int choose_chunk(const pilot_refine_handle* h, int n_hyp, int n_points) {
@@ -257,6 +292,7 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->chunk_override = 0;
   h->mode = PILOT_EXEC_AUTO;
   h->cluster_override = 0;
+  h->math_mode = PILOT_MATH_AUTO;
   h->last_launches = 0;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
   h->copy_stream = nullptr; h->n_submitted = h->n_waited = 0;
@@ -309,6 +345,12 @@ int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster) {
   if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return PILOT_ERR_ARG;
   h->mode = mode;
   h->cluster_override = cluster;
+  return PILOT_OK;
+}
+
+int pilot_refine_set_math_mode(pilot_refine_handle* h, int mode) {
+  if (!h || mode < PILOT_MATH_AUTO || mode > PILOT_MATH_MMA) return PILOT_ERR_ARG;
+  h->math_mode = mode;
   return PILOT_OK;
 }
 
@@ -384,15 +426,16 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
     const int g = lanes_per_unit(L.C, c.feat_dtype);
     const int cluster = choose_resident(h, A.n_hyp, L.N);
+    const bool mma = use_mma(h, g, p->grad_mode, cluster > 0);
     if (cluster > 0) {
-      if (resident_launch(c.feat_dtype, g, p->grad_mode, A, cluster, cuda_stream) != (int)cudaSuccess) {
+      if (resident_launch(c.feat_dtype, g, p->grad_mode, mma, A, cluster, cuda_stream) != (int)cudaSuccess) {
         if (prev != c.device) cudaSetDevice(prev);
         return PILOT_ERR_CUDA;
       }
       ++launches;
     } else {
-      pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode);
-      const size_t smem = gather_smem_for(g);
+      pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode, mma);
+      const size_t smem = gather_smem_for(g, mma);
       if (smem > 48 * 1024 && cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                    (int)smem) != cudaSuccess) {
         if (prev != c.device) cudaSetDevice(prev);

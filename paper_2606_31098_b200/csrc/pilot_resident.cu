@@ -32,7 +32,7 @@ struct ResidentShared {
   int go;
 };
 
-template <class T, int G, bool CEN>
+template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel(const __grid_constant__ PassArgs A) {
   cg::cluster_group cluster = cg::this_cluster();
   const unsigned S = cluster.num_blocks(), rank = cluster.block_rank();
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
     __syncthreads();
     if (!go) break;
 
-    PILOT_ZERO_ACC
+    acc_zero<MMA>(acc, sacc);
     if (prior_warp) {
       double rr = 0.0, Jr[6];
       const bool ok = range_prior(A, sh.pose, sh.pose + 9, lane, rr, Jr);
@@ -78,24 +78,13 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
         for (int i = 0; i < 6; ++i) sh.prior.J[i] = ok ? Jr[i] : 0.0;
       }
     } else {
-      photo_accumulate<T, G, CEN>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc, red);
+      photo_accumulate<T, G, CEN, MMA>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc, red);
     }
-    PILOT_LOAD_ACC
+    const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
 #ifdef PILOT_RESIDENT_PROFILE
     t_eval += clock64() - t0; t0 = clock64();
 #endif
-    // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
-#pragma unroll
-    for (int half = 16; half >= 1; half >>= 1) {
-      const bool upper = lane & half;
-#pragma unroll
-      for (int i = 0; i < half; ++i) {
-        float send = upper ? acc[i] : acc[i + half];
-        float keep = upper ? acc[i + half] : acc[i];
-        acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
-      }
-    }
-    sh.part[warp][lane] = acc[0];
+    sh.part[warp][lane] = wtot;
     __syncthreads();
     if (warp == 0) {
       float t = 0.f;
@@ -143,12 +132,35 @@ typedef void (*resident_fn)(const PassArgs);
 template <class T, bool CEN>
 resident_fn pick_g(int g) {
   switch (g) {
-    case 1: return lm_resident_kernel<T, 1, CEN>;
-    case 2: return lm_resident_kernel<T, 2, CEN>;
-    case 4: return lm_resident_kernel<T, 4, CEN>;
-    case 8: return lm_resident_kernel<T, 8, CEN>;
-    case 16: return lm_resident_kernel<T, 16, CEN>;
-    case 32: return lm_resident_kernel<T, 32, CEN>;
+#ifndef PILOT_FAST_BUILD
+    case 1: return lm_resident_kernel<T, 1, CEN, false>;
+#endif
+#ifndef PILOT_FAST_BUILD
+    case 2: return lm_resident_kernel<T, 2, CEN, false>;
+#endif
+    case 4: return lm_resident_kernel<T, 4, CEN, false>;
+    case 8: return lm_resident_kernel<T, 8, CEN, false>;
+#ifndef PILOT_FAST_BUILD
+    case 16: return lm_resident_kernel<T, 16, CEN, false>;
+#endif
+#ifndef PILOT_FAST_BUILD
+    case 32: return lm_resident_kernel<T, 32, CEN, false>;
+#endif
+  }
+  return nullptr;
+}
+
+template <class T>
+resident_fn pick_mma(int g) {
+  switch (g) {
+#ifndef PILOT_FAST_BUILD
+    case 2: return lm_resident_kernel<T, 2, false, true>;
+#endif
+    case 4: return lm_resident_kernel<T, 4, false, true>;
+    case 8: return lm_resident_kernel<T, 8, false, true>;
+#ifndef PILOT_FAST_BUILD
+    case 16: return lm_resident_kernel<T, 16, false, true>;
+#endif
   }
   return nullptr;
 }
@@ -156,25 +168,28 @@ resident_fn pick_g(int g) {
 template <bool CEN>
 resident_fn pick_t(pilot_dtype d, int g) {
   switch (d) {
+#ifndef PILOT_FAST_BUILD      /* tuning builds (-DPILOT_FAST_BUILD): bf16, 32 and 64 channels only */
     case PILOT_F32: return pick_g<F32Tag, CEN>(g);
-    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
     case PILOT_F16: return pick_g<F16Tag, CEN>(g);
+#endif
+    case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
   }
   return nullptr;
 }
 
 }  // namespace
 
-int pilot_internal::resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, const PassArgs& A, int cluster,
-                                    void* stream) {
-  resident_fn fn = grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(dtype, lanes_per_unit)
-                                                           : pick_t<false>(dtype, lanes_per_unit);
+int pilot_internal::resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, bool mma, const PassArgs& A,
+                                    int cluster, void* stream) {
+  resident_fn fn = mma ? (dtype == PILOT_BF16 ? pick_mma<BF16Tag>(lanes_per_unit) : pick_mma<F16Tag>(lanes_per_unit))
+                       : (grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(dtype, lanes_per_unit)
+                                                                  : pick_t<false>(dtype, lanes_per_unit));
   if (!fn || cluster < 1 || cluster > 8 || (cluster & (cluster - 1))) return (int)cudaErrorInvalidValue;
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof cfg);
   cfg.gridDim = dim3((unsigned)A.n_hyp * (unsigned)cluster, 1, 1);
   cfg.blockDim = dim3(kThreads, 1, 1);
-  const size_t smem = gather_smem_for(lanes_per_unit);
+  const size_t smem = gather_smem_for(lanes_per_unit, mma);
   if (smem > 48 * 1024 - 3 * 1024 &&
       cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return (int)cudaErrorInvalidValue;

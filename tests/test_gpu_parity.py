@@ -13,22 +13,27 @@ pytestmark = pytest.mark.gpu
 TOL = {"f32": (1e-4, 1e-3), "bf16": (5e-3, 5e-3), "f16": (5e-3, 5e-3)}
 
 
-MODE = {"mode": "passes", "cluster": 0}
+MODE = {"mode": "passes", "cluster": 0, "math": "auto"}
 
 
-@pytest.fixture(autouse=True, params=["passes", "split", "resident", "resident-c2", "resident-c8"])
+@pytest.fixture(autouse=True, params=["passes", "split", "resident", "resident-c2", "resident-c8", "passes-fp32",
+                                      "resident-fp32"])
 def exec_mode(request):
     """Every test of this file runs through both launch strategies (include/pilot_refine.h, pilot_exec_mode): one
-    launch per pass, and the cluster-resident kernel with the heuristic / 2 / 8 CTAs per hypothesis."""
+    launch per pass, and the cluster-resident kernel with the heuristic / 2 / 8 CTAs per hypothesis. They ask for the
+    tensor-core contraction (pilot_math_mode MMA), which is taken wherever it applies (16-bit features, 16-128
+    channels, exact bilinear gradient; FFMA2 elsewhere); the -fp32 variants force the FFMA2 contraction everywhere."""
     name = request.param
+    MODE["math"] = "fp32" if name.endswith("-fp32") else "mma"
+    name = name.replace("-fp32", "")
     MODE["mode"] = name.split("-")[0]
     MODE["cluster"] = int(name.split("-c")[1]) if "-c" in name else 0
-    yield name
+    yield request.param
 
 
 def gpu_refine(prob, params=None):
     from paper_2606_31098_b200 import binding
-    return binding.refine(prob, params, mode=MODE["mode"], cluster=MODE["cluster"])
+    return binding.refine(prob, params, mode=MODE["mode"], cluster=MODE["cluster"], math=MODE["math"])
 
 
 def both(prob, params=None):
@@ -101,7 +106,7 @@ def test_config1_teacher_forced_every_level(level):
     assert np.abs(gpu["n_valid"] - orc["n_valid"]).max() <= 1
 
 
-@pytest.mark.parametrize("dtype,C", [("f32", 4), ("f32", 8), ("f32", 32), ("bf16", 8), ("bf16", 16), ("bf16", 128),
+@pytest.mark.parametrize("dtype,C", [("f32", 4), ("f32", 8), ("f32", 32), ("bf16", 8), ("bf16", 16), ("bf16", 32), ("bf16", 64), ("bf16", 128),
                                       ("f16", 32), ("f16", 64), ("bf16", 256)])
 def test_lane_group_widths(dtype, C):
     """Every lanes-per-unit variant G = C*s/16 in {1..32}, with reference and query confidence weights."""
@@ -177,6 +182,7 @@ def test_host_path_matches_device_path():
     di = binding.DeviceInputs(prob, host=True)
     r = binding.Refiner.for_inputs(di, prob["params"], host_path=True)
     r.set_exec_mode(MODE["mode"], MODE["cluster"])
+    r.set_math_mode(MODE["math"])
     out = r.run(di, prob["params"])
     for k in ("poses", "cost", "iter_hessian"):
         assert np.array_equal(out[k].numpy(), dev[k]), k
@@ -192,7 +198,7 @@ def test_full_size_sampled_hypotheses(name, stride):
     if MODE["mode"] not in ("passes", "split"):
         pytest.skip("full sizes run in bench.py's launch configuration (AUTO = one launch per pass at these sizes)")
     prob = wl.make(name)
-    gpu = binding.refine(prob)
+    gpu = binding.refine(prob, math=MODE["math"])
     orc = po.run(po.Bound(prob), hyp_begin=0, hyp_step=stride, n_threads=8)
     idx = np.arange(0, prob["init_poses"].shape[0], stride)
     g = {k: (v[:, idx] if k.startswith("iter_") else v[idx]) for k, v in gpu.items() if isinstance(v, np.ndarray)}
@@ -261,6 +267,7 @@ def test_run_is_cuda_graph_capturable():
     di = binding.DeviceInputs(prob)
     r = binding.Refiner.for_inputs(di, prob["params"])
     r.set_exec_mode(MODE["mode"], MODE["cluster"])
+    r.set_math_mode(MODE["math"])
     eager = {k: v.clone() for k, v in r.run(di, prob["params"]).items()}
     torch.cuda.synchronize()
     side = torch.cuda.Stream()
@@ -285,6 +292,7 @@ def test_pipelined_host_path_matches_run_host():
     P = probs[0]["params"]
     r = binding.Refiner.for_inputs(his[0], P, host_path=True)
     r.set_exec_mode(MODE["mode"], MODE["cluster"])
+    r.set_math_mode(MODE["math"])
     want = []
     for hi in his:
         o = r.run(hi, P)
