@@ -92,6 +92,9 @@ struct PassArgs {
 // A.iters, A.rec_base): `cluster` CTAs per hypothesis. Returns a cudaError_t as int.
 int resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, bool mma, const PassArgs& A, int cluster, void* stream);
 
+// pilot_pass_mma.cu: one launch of the pass kernel with the tensor-core contraction (grid = A.n_hyp x A.n_chunks).
+int mma_pass_launch(pilot_dtype dtype, int lanes_per_unit, const PassArgs& A, void* stream);
+
 }  // namespace pilot_internal
 using namespace pilot_internal;
 
@@ -175,6 +178,15 @@ struct RawTaps { uint4 q00, q10, q01, q11, ref; };
 template <int PX>   // PX = bytes per pixel = 16*G: the x+1 taps are an immediate offset away
 __device__ __forceinline__ RawTaps load_taps(const char* feat, unsigned off, unsigned row_stride, const char* ref) {
   RawTaps t;
+#ifdef PILOT_PROBE_NO_LOADS
+  { const unsigned z = off >> 31, y = row_stride >> 31;     // zero, but not to the compiler
+    t.q00 = make_uint4(0x3f803f80u | z, 0x3f003f00u | y, 0x3e803f80u | z, 0x3f803e80u | y);
+    t.q10 = make_uint4(0x3f813f80u | y, 0x3f013f00u | z, 0x3e813f80u | y, 0x3f813e80u | z);
+    t.q01 = make_uint4(0x3f823f80u | z, 0x3f023f00u | z, 0x3e823f80u | y, 0x3f823e80u | y);
+    t.q11 = make_uint4(0x3f833f80u | y, 0x3f033f00u | y, 0x3e833f80u | z, 0x3f833e80u | z);
+    t.ref = make_uint4(0x3f843f80u | z, 0x3f043f00u | y, 0x3e843f80u | y, 0x3f843e80u | z); }
+  return t;
+#endif
   const char* p = feat + off;
   const char* q = p + row_stride;
   t.q00 = ldg16(p);
@@ -208,6 +220,11 @@ template <> __device__ __forceinline__ void unpack2<F16Tag>(const uint4& v, floa
 
 template <class T>
 __device__ __forceinline__ void unit_partials(const RawTaps& t, float a, float b, float (&p)[6]) {
+#ifdef PILOT_PROBE_LOADS_ONLY   /* tuning experiment: how fast is the gather alone (loads kept alive by an XOR fold) */
+  const unsigned x = t.q00.x ^ t.q10.y ^ t.q01.z ^ t.q11.w ^ t.ref.x ^ t.q00.w ^ t.q10.z ^ t.q01.y ^ t.q11.x ^ t.ref.y;
+  p[0] = (float)(x & 0x3ffu) * 1e-6f * a; p[1] = p[2] = p[3] = p[4] = 0.f; p[5] = b;
+  return;
+#endif
   constexpr int V2 = T::kVec / 2;
   float2 f00[V2], f10[V2], f01[V2], f11[V2], fr[V2];
   unpack2<T>(t.q00, f00); unpack2<T>(t.q10, f10); unpack2<T>(t.q01, f01); unpack2<T>(t.q11, f11);
@@ -368,14 +385,15 @@ template <> struct MmaType<F16Tag> {
 template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features stay on the FFMA2 path
 
 #ifndef PILOT_MMA_XBATCH
-#define PILOT_MMA_XBATCH 1      // 1: anchors and projection of the NEXT batch overlap the first taps of the current one
-                                // (config 4, prefetch 6: 12.57 ms without, 11.27 ms with)
+#define PILOT_MMA_XBATCH 0      // 1: anchors and projection of the NEXT batch overlap the first taps of the current one
+                                // (config 4 at 128 registers, prefetch 6: 12.57 ms without, 11.27 ms with; no room at 64)
 #endif
 #ifndef PILOT_MMA_SHFL_ACC
-#define PILOT_MMA_SHFL_ACC 0
+#define PILOT_MMA_SHFL_ACC 1      // 1: per-batch shuffle reduce-scatter into ONE accumulator register per lane (no
+                                  // shared-memory columns, no 29 live registers): what lets the kernel run at 64 registers
 #endif
 #ifndef PILOT_MMA_PREFETCH
-#define PILOT_MMA_PREFETCH 6    // rounds whose taps are in flight ahead of the tensor-core arithmetic
+#define PILOT_MMA_PREFETCH 2    // rounds whose taps are in flight ahead of the tensor-core arithmetic
 #endif
 
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
@@ -498,8 +516,13 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const int kap = g & (Geo::KH - 1), sel = (g >> Geo::LOGKH) & 1, uu = g >> (1 + Geo::LOGKH);
   const int u0 = uu * ROUNDS;
   const unsigned tofs = (unsigned)(kap * 64 + q * Geo::LB);
+#ifdef PILOT_PROBE_NODUP   /* tuning experiment (wrong arithmetic): sel 1 reads other lines than sel 0's f01 */
+  const char* pA = feat + tofs + (sel ? row_stride - 4u * PX : 0u);
+  const char* pF = feat + tofs + row_stride;
+#else
   const char* pA = feat + tofs + (sel ? row_stride : 0u);                 // + offset: f00 | f01;  + PX: f10 | f11
   const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
+#endif
   float* const srow = red + u0 * Geo::kStride + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
   bool useful; int js = 0;
   if constexpr (Geo::KH == 1) useful = q == uu;
@@ -809,7 +832,12 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
     }
 
     // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
+#ifdef PILOT_PROBE_NO_LIFT
+    if (valid) { PILOT_ACC(27) += cur[0] + cur[5]; PILOT_ACC(28) += 1.f; }
+    if (false) {
+#else
     if (valid) {
+#endif
       float wq = 1.f;
       if (L.conf) {
         const float* q = L.conf + (size_t)y0 * L.W + x0;

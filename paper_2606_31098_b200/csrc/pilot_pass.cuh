@@ -1,0 +1,61 @@
+// pilot_pass.cuh — the one-launch-per-pass photo kernel, shared by the two translation units
+// that instantiate it with different CTA shapes: pilot_refine.cu (FFMA2 contraction: 4 warps, 128 registers) and
+// pilot_pass_mma.cu (tensor-core contraction: 8 warps, 64 registers, 32 warps per SM). Shares no code with oracle/.
+#pragma once
+#include "pilot_device.cuh"
+
+namespace {
+
+template <class T, int G, bool CEN, bool MMA>
+__global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
+  const int m = blockIdx.x, chunk_idx = blockIdx.y;
+  const HypState* st = A.state + m;
+  if (st->level != A.level) return;             // finished this level early (failed factorisations)
+
+  PILOT_DECLARE_ACC
+  acc_zero<MMA>(acc, sacc);
+  {
+    const int begin = chunk_idx * A.chunk;
+    const double* Rc = st->Rc;
+    const double* Cc = st->Cc;
+    if constexpr (MMA) {                          // the tensor-core gather re-reads the pose from shared memory
+      __shared__ double s_pose[12];
+      if (threadIdx.x < 12) s_pose[threadIdx.x] = threadIdx.x < 9 ? st->Rc[threadIdx.x] : st->Cc[threadIdx.x - 9];
+      __syncthreads();
+      Rc = s_pose; Cc = s_pose + 9;
+    }
+    photo_accumulate<T, G, CEN, MMA>(A, Rc, Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc, red);
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
+  __shared__ float s_part[kWarps][kNacc];
+  __shared__ float s_sum[kNacc];
+  __shared__ int s_last;
+  s_part[warp][lane] = wtot;
+  __syncthreads();
+  if (warp == 0) {
+    float t = 0.f;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) t += s_part[w][lane];                    // fixed order
+    A.partials[((size_t)m * A.n_chunks + chunk_idx) * kNacc + lane] = t;
+    if (A.defer) return;                         // finalize_kernel (next launch) ends the iteration
+    __threadfence();
+    __syncwarp();
+    if (lane == 0) s_last = (atomicAdd(A.counters + m, 1u) == (unsigned)(A.n_chunks - 1));
+  }
+  if (A.defer) return;
+  __syncthreads();
+  if (!s_last || warp != 0) return;
+
+  // last CTA of this hypothesis: fixed-order sum over chunks (deterministic), then the LM step
+  __threadfence();
+  float t = 0.f;
+  const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
+  for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);
+  s_sum[lane] = t;
+  if (lane == 0) A.counters[m] = 0u;
+  __syncwarp();
+  finalize_in_workspace(A, m, s_sum, lane);
+}
+
+}  // namespace

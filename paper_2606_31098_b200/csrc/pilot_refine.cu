@@ -16,7 +16,7 @@
 #define PILOT_THREADS 128
 #define PILOT_MIN_BLOCKS 4
 #endif
-#include "pilot_device.cuh"
+#include "pilot_pass.cuh"
 
 #include <stdio.h>
 #include <string.h>
@@ -24,58 +24,6 @@
 namespace {
 
 // ------------------------------------------------------------------ kernels
-
-template <class T, int G, bool CEN, bool MMA>
-__global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
-  const int m = blockIdx.x, chunk_idx = blockIdx.y;
-  const HypState* st = A.state + m;
-  if (st->level != A.level) return;             // finished this level early (failed factorisations)
-
-  PILOT_DECLARE_ACC
-  acc_zero<MMA>(acc, sacc);
-  {
-    const int begin = chunk_idx * A.chunk;
-    const double* Rc = st->Rc;
-    const double* Cc = st->Cc;
-    if constexpr (MMA) {                          // the tensor-core gather re-reads the pose from shared memory
-      __shared__ double s_pose[12];
-      if (threadIdx.x < 12) s_pose[threadIdx.x] = threadIdx.x < 9 ? st->Rc[threadIdx.x] : st->Cc[threadIdx.x - 9];
-      __syncthreads();
-      Rc = s_pose; Cc = s_pose + 9;
-    }
-    photo_accumulate<T, G, CEN, MMA>(A, Rc, Cc, begin, min(begin + A.chunk, A.lv.N), (int)(threadIdx.x >> 5), kWarps, acc, sacc, red);
-  }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
-  __shared__ float s_part[kWarps][kNacc];
-  __shared__ float s_sum[kNacc];
-  __shared__ int s_last;
-  s_part[warp][lane] = wtot;
-  __syncthreads();
-  if (warp == 0) {
-    float t = 0.f;
-#pragma unroll
-    for (int w = 0; w < kWarps; ++w) t += s_part[w][lane];                    // fixed order
-    A.partials[((size_t)m * A.n_chunks + chunk_idx) * kNacc + lane] = t;
-    if (A.defer) return;                         // finalize_kernel (next launch) ends the iteration
-    __threadfence();
-    __syncwarp();
-    if (lane == 0) s_last = (atomicAdd(A.counters + m, 1u) == (unsigned)(A.n_chunks - 1));
-  }
-  if (A.defer) return;
-  __syncthreads();
-  if (!s_last || warp != 0) return;
-
-  // last CTA of this hypothesis: fixed-order sum over chunks (deterministic), then the LM step
-  __threadfence();
-  float t = 0.f;
-  const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
-  for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);
-  s_sum[lane] = t;
-  if (lane == 0) A.counters[m] = 0u;
-  __syncwarp();
-  finalize_in_workspace(A, m, s_sum, lane);
-}
 
 // Deferred finalisation: one WARP per hypothesis. With many hypotheses and few anchors each (the paper's coarse level:
 // 1210 x 500) every CTA of the pass kernel would end in the serial fp64 tail while holding an SM slot that waiting CTAs
@@ -199,21 +147,6 @@ pass_fn pick_g(int g) {
   return nullptr;
 }
 
-template <class T>
-pass_fn pick_mma(int g) {
-  switch (g) {
-#ifndef PILOT_FAST_BUILD
-    case 2: return photo_pass_kernel<T, 2, false, true>;
-#endif
-    case 4: return photo_pass_kernel<T, 4, false, true>;
-    case 8: return photo_pass_kernel<T, 8, false, true>;
-#ifndef PILOT_FAST_BUILD
-    case 16: return photo_pass_kernel<T, 16, false, true>;
-#endif
-  }
-  return nullptr;
-}
-
 template <bool CEN>
 pass_fn pick_t(pilot_dtype d, int g) {
   switch (d) {
@@ -226,8 +159,7 @@ pass_fn pick_t(pilot_dtype d, int g) {
   return nullptr;
 }
 
-pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode, bool mma) {
-  if (mma) return d == PILOT_BF16 ? pick_mma<BF16Tag>(g) : pick_mma<F16Tag>(g);
+pass_fn pick_kernel(pilot_dtype d, int g, int grad_mode) {
   return grad_mode == PILOT_GRAD_CENTRAL_SAMPLED ? pick_t<true>(d, g) : pick_t<false>(d, g);
 }
 
@@ -251,8 +183,8 @@ bool use_mma(const pilot_refine_handle* h, int g, int grad_mode, bool resident) 
   if (h->math_mode == PILOT_MATH_FP32) return false;
   const bool applies = h->cfg.feat_dtype != PILOT_F32 && grad_mode == PILOT_GRAD_BILINEAR_EXACT && (g == 2 || g == 4 || g == 8 || g == 16);
   if (h->math_mode == PILOT_MATH_MMA) return applies;
-  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.93 -> 11.27, config 2 11.46 -> 10.90 (64 channels, one
-  // launch per pass); config 1 0.67 -> 0.75, config 3 1.12 -> 1.24, paper schedule 0.32 -> 0.34 (32 channels, cluster-resident)
+  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.89 -> 10.29, config 2 11.43 -> 9.76 (64 channels, one
+  // launch per pass); config 1 0.67 -> 0.72, config 3 1.12 -> 1.20, paper schedule 0.32 -> 0.33 (32 channels, cluster-resident)
   return applies && g >= 8 && !resident;
 }
 
@@ -421,12 +353,13 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     L.fx = in->intrinsics[l][0]; L.fy = in->intrinsics[l][1]; L.cx = in->intrinsics[l][2]; L.cy = in->intrinsics[l][3];
     L.W = c.width[l]; L.H = c.height[l]; L.C = c.channels[l]; L.N = in->n_points[l];
     A.level = l; A.iters = p->iters[l]; A.rec_base = rec_base;
-    A.chunk = choose_chunk(h, A.n_hyp, L.N);
-    A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
-    if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
     const int g = lanes_per_unit(L.C, c.feat_dtype);
     const int cluster = choose_resident(h, A.n_hyp, L.N);
     const bool mma = use_mma(h, g, p->grad_mode, cluster > 0);
+    A.chunk = choose_chunk(h, A.n_hyp, L.N);
+    if (mma && cluster == 0 && A.chunk < 2 * kMinChunk) A.chunk = 2 * kMinChunk;      // its CTAs have 8 warps: one batch per warp
+    A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
+    if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
     if (cluster > 0) {
       if (resident_launch(c.feat_dtype, g, p->grad_mode, mma, A, cluster, cuda_stream) != (int)cudaSuccess) {
         if (prev != c.device) cudaSetDevice(prev);
@@ -434,10 +367,10 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
       }
       ++launches;
     } else {
-      pass_fn fn = pick_kernel(c.feat_dtype, g, p->grad_mode, mma);
-      const size_t smem = gather_smem_for(g, mma);
-      if (smem > 48 * 1024 && cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                   (int)smem) != cudaSuccess) {
+      pass_fn fn = mma ? nullptr : pick_kernel(c.feat_dtype, g, p->grad_mode);
+      const size_t smem = mma ? 0 : gather_smem_for(g, false);
+      if (!mma && smem > 48 * 1024 && cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                           (int)smem) != cudaSuccess) {
         if (prev != c.device) cudaSetDevice(prev);
         return PILOT_ERR_CUDA;
       }
@@ -450,7 +383,14 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
                  ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 512));
       for (int pass = 0; pass <= p->iters[l]; ++pass) {
         A.pass = pass;
-        fn<<<grid, kThreads, smem, st>>>(A);
+        if (mma) {
+          if (mma_pass_launch(c.feat_dtype, g, A, cuda_stream) != (int)cudaSuccess) {
+            if (prev != c.device) cudaSetDevice(prev);
+            return PILOT_ERR_CUDA;
+          }
+        } else {
+          fn<<<grid, kThreads, smem, st>>>(A);
+        }
         ++launches;
         if (A.defer) {
           finalize_kernel<<<(A.n_hyp + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(A);
