@@ -392,16 +392,22 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
 #define PILOT_MMA_SHFL_ACC 1      // 1: per-batch shuffle reduce-scatter into ONE accumulator register per lane (no
                                   // shared-memory columns, no 29 live registers): what lets the kernel run at 64 registers
 #endif
-#ifndef PILOT_MMA_PREFETCH
-#define PILOT_MMA_PREFETCH 2    // rounds whose taps are in flight ahead of the tensor-core arithmetic
+#ifndef PILOT_MMA_PREFETCH_REGS
+#define PILOT_MMA_PREFETCH_REGS 24   // registers of taps in flight ahead of the tensor-core arithmetic: 1 round of 32-byte
+                                     // loads, 2 rounds of 16-byte loads (one round = three loads per thread)
+#endif
+#ifndef PILOT_MMA_LB32
+#define PILOT_MMA_LB32 1        // 1: 64 and more channels use 32-byte loads (LDG.256): half the load instructions and rounds
 #endif
 
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
-  static constexpr int KS = CH >= 32 ? 2 : 1;          // k-steps of 16 channels per mma chain
-  static constexpr int KH = CH >= 32 ? CH / 32 : 1;    // 32-channel slices per pixel
+  static constexpr int LBMAX = PILOT_MMA_LB32 ? 32 : 16;
+  static constexpr int LB = CH / 2 < LBMAX ? CH / 2 : LBMAX;   // bytes per load per thread (the 4 q-threads share a slice)
+  static constexpr int NW = LB / 4;                    // 32-bit words (= pairs of channels) per load per thread
+  static constexpr int KS = NW / 2;                    // k-steps of 16 channels per mma chain
+  static constexpr int SLICE = 4 * LB;                 // bytes of a pixel that one row-group covers
+  static constexpr int KH = 2 * CH / SLICE;            // slices per pixel
   static constexpr int LOGKH = KH == 4 ? 2 : (KH == 2 ? 1 : 0);
-  static constexpr int NW = 2 * KS;                    // 32-bit words (= pairs of channels) per load per thread
-  static constexpr int LB = 4 * NW;                    // bytes per load per thread
   static constexpr int UR = 4 / KH;                    // units per round
   static constexpr int ROUNDS = 32 / UR;
   static constexpr int PX = CH * 2;                    // bytes per pixel
@@ -414,7 +420,10 @@ template <int G> __host__ __device__ constexpr bool mma_supported() { return G =
 template <int NW> struct TapWords { unsigned w[NW]; };
 template <int NW> __device__ __forceinline__ TapWords<NW> ldg_words(const char* p) {
   TapWords<NW> t;
-  if constexpr (NW == 4) {
+  if constexpr (NW == 8) {                     // 32-byte load (sm_100: LDG.256); p is 32-byte aligned
+    asm("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=r"(t.w[0]), "=r"(t.w[1]), "=r"(t.w[2]), "=r"(t.w[3]), "=r"(t.w[4]), "=r"(t.w[5]), "=r"(t.w[6]), "=r"(t.w[7]) : "l"(p));
+  } else if constexpr (NW == 4) {
     const uint4 v = ldg16(p);
     t.w[0] = v.x; t.w[1] = v.y; t.w[2] = v.z; t.w[3] = v.w;
   } else {
@@ -480,7 +489,7 @@ template <int G, bool MMA> constexpr size_t gather_smem_bytes() {
 //   lane-per-unit   anchor load, projection + visibility in fp64 (a2) - done ONE BATCH AHEAD, while the first taps
 //                   of the current batch are in flight, so that the tap latency at the head of a batch is covered;
 //   fragment roles  ROUNDS rounds of (HSUB2 differences -> 2 KS mma.sync) over UR units each, taps prefetched
-//                   PILOT_MMA_PREFETCH rounds ahead; the 4 x 4 diagonal blocks go to the warp's buffer `red`;
+//                   PILOT_MMA_PREFETCH_REGS registers ahead; the 4 x 4 diagonal blocks go to the warp's buffer `red`;
 //   lane-per-unit   Gram -> six scalars, robust weight, lift through J_uv, accumulate (a4-a6).
 template <class T, int G>
 __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const double* Rc, const double* Ccand,
@@ -495,17 +504,17 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   using Geo = MmaGeom<CH>;
   using M = MmaType<T>;
   constexpr int NW = Geo::NW, PX = Geo::PX, ROUNDS = Geo::ROUNDS;
-  constexpr int PF = PILOT_MMA_PREFETCH < ROUNDS ? PILOT_MMA_PREFETCH : ROUNDS;
+  constexpr int PFW = PILOT_MMA_PREFETCH_REGS / (3 * NW) < 1 ? 1 : PILOT_MMA_PREFETCH_REGS / (3 * NW);
+  constexpr int PF = PFW < ROUNDS ? PFW : ROUNDS;
   const LevelArgs& L = A.lv;
   const int lane = threadIdx.x & 31;
   const unsigned row_stride = (unsigned)PX * (unsigned)L.W;
   const char* feat = static_cast<const char*>(L.feat);
   const char* refb = static_cast<const char*>(L.ref);
 
-  // The candidate pose stays in SHARED memory (Rc, Ccand must point there) and is re-read by every projection: as 24
+  // The candidate pose stays in SHARED memory (Rc[9] and Ccand = Rc + 9 must point there, 16-byte aligned) and is re-read by every projection: as 24
   // registers held across the rounds it forced the address arithmetic of every round to be rematerialised.
-  const volatile double* R = Rc;
-  const volatile double* Cc = Ccand;
+  const unsigned pose_s = (unsigned)__cvta_generic_to_shared(Rc);         // Rc[9] | Cc[3] contiguous, 16-byte aligned
   const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
 
   // fragment roles: g = (uu, sel, slice), slice in the low bits: the 8 lanes of a quarter-warp (one phase of a 16-byte
@@ -515,7 +524,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const int q = lane & 3, g = lane >> 2;
   const int kap = g & (Geo::KH - 1), sel = (g >> Geo::LOGKH) & 1, uu = g >> (1 + Geo::LOGKH);
   const int u0 = uu * ROUNDS;
-  const unsigned tofs = (unsigned)(kap * 64 + q * Geo::LB);
+  const unsigned tofs = (unsigned)(kap * Geo::SLICE + q * Geo::LB);
 #ifdef PILOT_PROBE_NODUP   /* tuning experiment (wrong arithmetic): sel 1 reads other lines than sel 0's f01 */
   const char* pA = feat + tofs + (sel ? row_stride - 4u * PX : 0u);
   const char* pF = feat + tofs + row_stride;
@@ -534,6 +543,11 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   auto project = [&](const float4& P, int base) {                         // a2, in double so that u, v carry no fp32 noise
     Unit U;
     bool valid = base + lane < end;
+    double R[12];                                                         // six 16-byte shared-memory loads
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+      asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
+    const double* Cc = R + 9;
     double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
     double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
     double Yd = R[3] * dx + R[4] * dy + R[5] * dz;

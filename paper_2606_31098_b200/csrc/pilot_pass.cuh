@@ -1,6 +1,6 @@
 // pilot_pass.cuh — the one-launch-per-pass photo kernel, shared by the two translation units
 // that instantiate it with different CTA shapes: pilot_refine.cu (FFMA2 contraction: 4 warps, 128 registers) and
-// pilot_pass_mma.cu (tensor-core contraction: 8 warps, 64 registers, 32 warps per SM). Shares no code with oracle/.
+// pilot_pass_mma.cu (tensor-core contraction: 4 warps, 72 registers, 28 warps per SM). Shares no code with oracle/.
 #pragma once
 #include "pilot_device.cuh"
 
@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
     const double* Rc = st->Rc;
     const double* Cc = st->Cc;
     if constexpr (MMA) {                          // the tensor-core gather re-reads the pose from shared memory
-      __shared__ double s_pose[12];
+      __shared__ __align__(16) double s_pose[12];
       if (threadIdx.x < 12) s_pose[threadIdx.x] = threadIdx.x < 9 ? st->Rc[threadIdx.x] : st->Cc[threadIdx.x - 9];
       __syncthreads();
       Rc = s_pose; Cc = s_pose + 9;

@@ -1,11 +1,16 @@
 // pilot_pass_mma.cu — the pass kernel with the tensor-core contraction (pilot_math_mode MMA), in a translation unit of
-// its own because its CTA shape differs: 8 warps at 64 registers, 4 CTAs = 32 warps per SM. The gather is bound by
-// load latency and the L1 data path, not by issue slots, once the contraction is on the tensor cores; measured on
-// config 4 (B200, ms per step): 16 warps per SM at 128 registers with 6 rounds of taps in flight 11.27, 32 warps at
-// 64 registers with 2 rounds in flight 10.29 (FFMA2 path: 11.93).
+// its own because its CTA shape differs: 4 warps at 72 registers, 7 CTAs = 28 warps per SM. Once the contraction is on
+// the tensor cores the gather is bound by load latency and by the L1 data path (85 % busy), not by issue slots, and
+// warps hide that better than registers of prefetched taps; measured on config 4 (B200, ms per step): 16 warps per SM at
+// 128 registers with 6 rounds of 16-byte taps in flight 11.27; 32 warps at 64 registers with 2 rounds in flight 10.29;
+// 32-byte loads (LDG.256, half the rounds), 28 warps at 72 registers, 1 round in flight 9.60 (FFMA2 path: 11.89).
 // Shares no code with oracle/.
-#define PILOT_THREADS 256
-#define PILOT_MIN_BLOCKS 4
+#ifndef PILOT_MMA_THREADS
+#define PILOT_MMA_THREADS 128
+#define PILOT_MMA_MIN_BLOCKS 7
+#endif
+#define PILOT_THREADS PILOT_MMA_THREADS
+#define PILOT_MIN_BLOCKS PILOT_MMA_MIN_BLOCKS
 #include "pilot_pass.cuh"
 
 namespace {

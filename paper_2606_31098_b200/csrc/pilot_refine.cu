@@ -183,7 +183,7 @@ bool use_mma(const pilot_refine_handle* h, int g, int grad_mode, bool resident) 
   if (h->math_mode == PILOT_MATH_FP32) return false;
   const bool applies = h->cfg.feat_dtype != PILOT_F32 && grad_mode == PILOT_GRAD_BILINEAR_EXACT && (g == 2 || g == 4 || g == 8 || g == 16);
   if (h->math_mode == PILOT_MATH_MMA) return applies;
-  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.89 -> 10.29, config 2 11.43 -> 9.76 (64 channels, one
+  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.89 -> 9.60, config 2 11.43 -> 9.61 (64 channels, one
   // launch per pass); config 1 0.67 -> 0.72, config 3 1.12 -> 1.20, paper schedule 0.32 -> 0.33 (32 channels, cluster-resident)
   return applies && g >= 8 && !resident;
 }
@@ -355,9 +355,9 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     A.level = l; A.iters = p->iters[l]; A.rec_base = rec_base;
     const int g = lanes_per_unit(L.C, c.feat_dtype);
     const int cluster = choose_resident(h, A.n_hyp, L.N);
-    const bool mma = use_mma(h, g, p->grad_mode, cluster > 0);
+    bool mma = use_mma(h, g, p->grad_mode, cluster > 0);
+    if (mma && MmaGeom<64>::LB == 32 && g >= 8 && (((uintptr_t)L.feat | (uintptr_t)L.ref) & 31)) mma = false;   // 32-byte loads
     A.chunk = choose_chunk(h, A.n_hyp, L.N);
-    if (mma && cluster == 0 && A.chunk < 2 * kMinChunk) A.chunk = 2 * kMinChunk;      // its CTAs have 8 warps: one batch per warp
     A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
     if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
     if (cluster > 0) {

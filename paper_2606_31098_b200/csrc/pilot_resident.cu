@@ -24,7 +24,7 @@ namespace {
 
 struct ResidentShared {
   HypState st;                       // rank 0: the hypothesis' optimiser state for the whole level
-  double pose[12];                   // this CTA's copy of the candidate pose: Rc[9], Cc[3]
+  __align__(16) double pose[12];     // this CTA's copy of the candidate pose: Rc[9], Cc[3]
   float part[kWarps][kNacc];
   float cta_sum[kNacc];              // this CTA's slice total; rank 0 reads it through DSMEM
   float tot[kNacc];
