@@ -24,8 +24,28 @@ UNIT = "point-hyp-iters/s"
 LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", "iter_cost", "iter_lambda")
 
 # dram__bytes_read.sum + dram__bytes_write.sum per photo_pass_kernel launch from the committed `ncu --set full`
-# capture of this command (profiles/r1d_photo_config4.md); None where no capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"config4": 35.3e6}
+# capture of this command (profiles/r1e_photo_config4.md; r1d for --math fp32: the same 34-37 MB); None where no
+# capture of that workload exists.
+NCU_TRAFFIC_BYTES = {"config4": 35.5e6}
+# From the same captures, per (anchor, hypothesis) unit-evaluation of the pass kernel at C = 64 bf16: warp instructions
+# and L1 data-pipe wavefronts (l1tex__data_pipe_lsu_wavefronts: global + shared + local + shuffles). C = 32: the
+# cluster-resident kernel (profiles/r1c_resident_small_workloads.md).
+NCU_PER_UNIT = {("mma", 64): {"inst": 29.2, "l1_wavefronts": 12.2, "source": "profiles/r1e_photo_config4.md"},
+                ("fp32", 64): {"inst": 47.5, "l1_wavefronts": 11.4, "source": "profiles/r1d_photo_config4.md"},
+                ("fp32", 32): {"inst": 32.7, "l1_wavefronts": None, "source": "profiles/r1c_resident_small_workloads.md"}}
+
+
+def contraction_used(args, prob, H):
+    """Which per-unit contraction the library takes for this run (pilot_math_mode, include/pilot_refine.h): mirrors
+    AUTO's rule so that the roofline constants match the kernel that ran."""
+    C, N = prob["channels"][-1], max(p.shape[0] for p in prob["points"])
+    applies = prob["dtype"] != "f32" and C in (16, 32, 64, 128)
+    if args.math == "fp32" or not applies:
+        return "fp32"
+    if args.math == "mma":
+        return "mma"
+    resident = args.mode == "resident" or (args.mode == "auto" and H * N <= 1500000 and H <= 296)
+    return "mma" if C >= 64 and not resident else "fp32"
 
 
 def load_peaks():
@@ -488,22 +508,39 @@ def main():
     flops_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2)) \
         * 2 * (19 * W.prob["channels"][-1] + 120)
     alu_peak = prop.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
+    contraction = contraction_used(args, W.prob, getattr(W, "H", None) or getattr(W, "keep", 1))
+    roofline["contraction"] = contraction
     roofline["alu"] = {"bound": "alu", "achieved": flops_per_launch / launch_s / 1e12, "peak": alu_peak,
                        "unit": "TFLOP/s", "frac": flops_per_launch / launch_s / 1e12 / alu_peak,
                        "note": "fp32 FMA lanes: 2*(19*C+120) algorithmic flop per unit-evaluation against "
-                               "SMs*128*2*1.965 GHz; the kernel is issue/FMA-pipe bound, not byte bound "
-                               "(profiles/r1d_photo_config4.md)"}
+                               "SMs*128*2*1.965 GHz. With the FFMA2 contraction the kernel is issue/FMA-pipe bound "
+                               "(profiles/r1d_photo_config4.md); with the tensor-core contraction the 19*C part runs as "
+                               "mma.sync and the L1 data pipe binds instead (roofline.l1)"}
+    per_unit = NCU_PER_UNIT.get((contraction, W.prob["channels"][-1])) if W.prob["dtype"] != "f32" else None
+    units_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2))
+    if per_unit and per_unit["l1_wavefronts"]:
+        # the unit that binds (profiles/r1e_photo_config4.md): the LSU data pipe moves one 128-byte wavefront per
+        # clock per SM; wavefronts per unit come from the committed ncu capture, the time from this run
+        l1_peak = prop.multi_processor_count * 1.965e9
+        l1_rate = units_per_launch * per_unit["l1_wavefronts"] / launch_s
+        roofline["l1"] = {"bound": "l1-data-pipe", "achieved": l1_rate / 1e9, "peak": l1_peak / 1e9, "unit": "Gwavefront/s",
+                          "frac": l1_rate / l1_peak, "wavefronts_per_unit": per_unit["l1_wavefronts"],
+                          "algorithmic_wavefronts_per_unit": (4 * W.prob["channels"][-1] * 2 + W.prob["channels"][-1] * 2) / 128.0,
+                          "source": per_unit["source"],
+                          "note": "l1tex__data_pipe_lsu_wavefronts per unit (global + shared + shuffles + local) x units "
+                                  "per launch / launch time against SMs x 1 wavefront/clk x 1.965 GHz; the algorithmic "
+                                  "floor is the 4 taps + the reference row (5 x 128 B at C = 64 bf16)"}
     # t_model = max(compulsory HBM bytes / HBM peak, gather bytes / L2 gather peak, flops / FMA
     # peak); the L2 term is filled in below when the probe runs. Instruction issue (warp instructions per unit from
     # the committed ncu captures) is listed beside it because it is the term that binds.
     compulsory = float(map_bytes) / max(1, W.prob["n_levels"])          # one level's map read once per pass
     model = {"t_hbm_compulsory_ms": compulsory / (peak * 1e9) * 1e3, "t_fma_ms": flops_per_launch / (alu_peak * 1e12) * 1e3,
              "t_l2_gather_ms": None, "t_run_ms": launch_s * 1e3}
-    inst_per_unit = {64: 47.5, 32: 32.7}.get(W.prob["channels"][-1]) if W.prob["dtype"] != "f32" else None
-    if inst_per_unit:
-        units_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * 2)
-        model["t_issue_ms"] = units_per_launch * inst_per_unit / (prop.multi_processor_count * 4 * 1.965e9) * 1e3
-        model["issue_source"] = "warp instructions per unit from profiles/r1d_photo_config4.md (C=64) / r1c_resident_small_workloads.md (C=32)"
+    if per_unit:
+        model["t_issue_ms"] = units_per_launch * per_unit["inst"] / (prop.multi_processor_count * 4 * 1.965e9) * 1e3
+        model["issue_source"] = "warp instructions per unit from " + per_unit["source"]
+        if per_unit["l1_wavefronts"]:
+            model["t_l1_pipe_ms"] = units_per_launch * per_unit["l1_wavefronts"] / (prop.multi_processor_count * 1.965e9) * 1e3
     roofline["model"] = model
     if rank == 0 and not args.no_probe:
         # the build's own micro-benchmark: random gathers with the kernel's access shape
@@ -549,7 +586,9 @@ def main():
                                 "all-gather + arg-min ends the step when n_gpus > 1"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+                "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if contraction == "fp32" else W.prob["dtype"] + " mma.sync products, f32 accumulate; f32 elsewhere",
+                "data": "synthetic", "config": cfg,
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
                 "gpu_launches": int(launches_per_step * args.steps), "clocks": sampler.summary()}
         print(json.dumps(line))

@@ -2,8 +2,11 @@
 // vec_bytes (one bilinear tap of C channels: 64 B for C=32 bf16, 128 B for C=64 bf16; 256/512 B for a whole
 // 2x2 footprint) from a buffer that is either L2-resident or much larger than L2. It gives the denominators the
 // photo kernel's gather is compared with: the L2->SM random-gather peak and the HBM random-gather peak (which is
-// below the streaming-copy peak of MEASURED_PEAKS.json). Same access shape as the kernel: 16-byte ld.global.nc
-// per lane, the vec_bytes/16 lanes of a group reading one contiguous vector.
+// below the streaming-copy peak of MEASURED_PEAKS.json). Same access shapes as the kernels: 16-byte ld.global.nc per
+// lane (FFMA2 gather) and, for vectors of 64 bytes and more, 32-byte loads (LDG.256, the tensor-core gather); the
+// vec_bytes/16 or /32 lanes of a group read one contiguous vector. The result is the better of the two: the LSU costs
+// per load instruction up to 32 bytes per lane, so the wider load sets the ceiling (measured: 14.4 vs 16.8 TB/s from
+// an L2-resident buffer).
 #include "../../include/pilot_refine.h"
 
 #include <cuda_runtime.h>
@@ -16,8 +19,18 @@ __device__ __forceinline__ uint32_t mix(uint32_t x) {          // counter-based 
   return x;
 }
 
-template <int UNROLL>
-__global__ void __launch_bounds__(256) gather_probe_kernel(const uint4* __restrict__ buf, uint32_t n_vec, int lanes_per_vec,
+// WB = bytes per lane per load: 16 (LDG.128) or 32 (LDG.256)
+template <int WB> __device__ __forceinline__ uint4 probe_load(const char* p);
+template <> __device__ __forceinline__ uint4 probe_load<16>(const char* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+template <> __device__ __forceinline__ uint4 probe_load<32>(const char* p) {
+  uint4 a, b;
+  asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+  return make_uint4(a.x ^ b.x, a.y ^ b.y, a.z ^ b.z, a.w ^ b.w);
+}
+
+template <int UNROLL, int WB>
+__global__ void __launch_bounds__(256) gather_probe_kernel(const char* __restrict__ buf, uint32_t n_vec, int lanes_per_vec,
                                                            uint32_t vecs_per_thread_group, uint32_t seed, uint4* sink) {
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t group = tid / lanes_per_vec, sub = tid % lanes_per_vec;
@@ -27,7 +40,7 @@ __global__ void __launch_bounds__(256) gather_probe_kernel(const uint4* __restri
 #pragma unroll
     for (int u = 0; u < UNROLL; ++u) {
       uint32_t k = mix((group * vecs_per_thread_group + i + u) ^ seed) % n_vec;
-      v[u] = __ldg(buf + (size_t)k * lanes_per_vec + sub);
+      v[u] = probe_load<WB>(buf + ((size_t)k * lanes_per_vec + sub) * WB);
     }
 #pragma unroll
     for (int u = 0; u < UNROLL; ++u) { acc.x ^= v[u].x; acc.y ^= v[u].y; acc.z ^= v[u].z; acc.w ^= v[u].w; }
@@ -48,7 +61,6 @@ int pilot_refine_probe_gather(int device, size_t buffer_bytes, int vec_bytes, in
   if (cudaSetDevice(device) != cudaSuccess) return PILOT_ERR_CUDA;
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaSetDevice(prev); return PILOT_ERR_CUDA; }
-  const int lanes = vec_bytes / 16;
   const size_t n_vec = buffer_bytes / vec_bytes;
   void *buf = nullptr, *sink = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -59,17 +71,25 @@ int pilot_refine_probe_gather(int device, size_t buffer_bytes, int vec_bytes, in
   if (ok) {
     const int ctas = prop.multiProcessorCount * 8;                 // 8 resident CTAs of 256 threads per SM
     const uint32_t per_group = 256;                                // vectors per lane group per launch
-    const double bytes = (double)ctas * 256 / lanes * per_group * vec_bytes;
-    for (int it = 0; it < launches + 2 && ok; ++it) {              // 2 warm-up launches (also fill L2 when it fits)
-      cudaEventRecord(e0);
-      gather_probe_kernel<8><<<ctas, 256>>>(static_cast<const uint4*>(buf), (uint32_t)n_vec, lanes, per_group,
-                                           0x9e3779b9u * (uint32_t)(it + 1), static_cast<uint4*>(sink));
-      cudaEventRecord(e1);
-      ok = cudaEventSynchronize(e1) == cudaSuccess && cudaGetLastError() == cudaSuccess;
-      float ms = 0.f;
-      if (ok && it >= 2 && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess && ms > 0.f) {
-        double g = bytes / (ms * 1e-3) / 1e9;
-        if (g > best) best = g;
+    for (int wb = 16; wb <= (vec_bytes >= 64 ? 32 : 16) && ok; wb *= 2) {
+      const int lanes = vec_bytes / wb;
+      const double bytes = (double)ctas * 256 / lanes * per_group * vec_bytes;
+      for (int it = 0; it < launches + 2 && ok; ++it) {            // 2 warm-up launches (also fill L2 when it fits)
+        cudaEventRecord(e0);
+        const uint32_t seed = 0x9e3779b9u * (uint32_t)(it + 1);
+        if (wb == 16)
+          gather_probe_kernel<8, 16><<<ctas, 256>>>(static_cast<const char*>(buf), (uint32_t)n_vec, lanes, per_group, seed,
+                                                    static_cast<uint4*>(sink));
+        else
+          gather_probe_kernel<8, 32><<<ctas, 256>>>(static_cast<const char*>(buf), (uint32_t)n_vec, lanes, per_group, seed,
+                                                    static_cast<uint4*>(sink));
+        cudaEventRecord(e1);
+        ok = cudaEventSynchronize(e1) == cudaSuccess && cudaGetLastError() == cudaSuccess;
+        float ms = 0.f;
+        if (ok && it >= 2 && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess && ms > 0.f) {
+          double g = bytes / (ms * 1e-3) / 1e9;
+          if (g > best) best = g;
+        }
       }
     }
   }

@@ -313,3 +313,75 @@ def test_pipelined_host_path_matches_run_host():
             assert np.array_equal(got[k][n].numpy(), want[k % 2][n].numpy()), (k, n)
     assert not np.array_equal(want[0]["poses"].numpy(), want[1]["poses"].numpy())
     r.close()
+
+
+# ------------------------------------------------------------------ tensor-core contraction (pilot_math_mode MMA)
+
+def _both_contractions(prob, P=None):
+    from oracle import pilot_oracle as po
+    from paper_2606_31098_b200 import binding
+    PP = dict(prob.get("params", {})); PP.update(P or {})
+    m = binding.refine(prob, PP, mode=MODE["mode"], cluster=MODE["cluster"], math="mma")
+    f = binding.refine(prob, PP, mode=MODE["mode"], cluster=MODE["cluster"], math="fp32")
+    return m, f, po.run(po.Bound(prob, PP), n_threads=8)
+
+
+@pytest.mark.parametrize("dtype,level", [("bf16", 1e-3), ("f16", 2e-4)])
+@pytest.mark.parametrize("C", [16, 32, 64, 128])
+@pytest.mark.parametrize("smooth", [False, True])
+def test_tensor_core_contraction_error_level(dtype, level, C, smooth):
+    """The first differences of the tensor-core path are rounded once in the storage type wherever the two taps are
+    not within a factor of two of each other. On a white-noise map (smooth=False: every difference is rounded) H, g
+    and the cost stay a decade inside north_star's 5e-3 (measured: bf16 6e-5 .. 3e-4, fp16 ~1e-5; the FFMA2 path sits
+    at fp32 rounding, 1e-7); `level` pins that so that a regression of the arithmetic shows up before the tolerance."""
+    if MODE["math"] == "fp32":
+        pytest.skip("runs both contractions itself")
+    prob = tiny(seed=41, N=900, C=C, n_hyp=4, dtype=dtype, W=64, H=48, smooth=smooth)
+    m, f, o = _both_contractions(prob, dict(iters=[2], loss="huber", loss_scale=0.5, min_valid=4))
+    em, ef = parity.system_errors(m, o, 0), parity.system_errors(f, o, 0)        # record 0: the system at the input pose
+    assert max(e.max() for e in em) <= level, [e.max() for e in em]
+    assert max(e.max() for e in ef) <= 1e-5, [e.max() for e in ef]
+    em1 = parity.system_errors(m, o, 1)                                          # record 1: each side at its own iterate
+    assert max(e.max() for e in em1) <= TOL[dtype][0], [e.max() for e in em1]
+    assert np.array_equal(m["n_valid"], o["n_valid"]) and np.array_equal(f["n_valid"], o["n_valid"])
+
+
+def test_tensor_core_contraction_smooth_config4_recipe():
+    """config 4's recipe at a reduced size (smooth band-limited map, sigma = 0.02 reference noise): neighbouring taps
+    are within a factor of two almost everywhere, so most differences are exact (measured: H 2e-5, g 7e-6)."""
+    if MODE["math"] == "fp32":
+        pytest.skip("runs both contractions itself")
+    prob = wl.config4(H=6, N=3000, iters=2, width=480, height=270, dsm_size=1024)
+    m, f, o = _both_contractions(prob)
+    em = parity.system_errors(m, o, 0)
+    assert max(e.max() for e in em) <= 2e-4, [e.max() for e in em]
+    Tm, Tf = m["poses"].reshape(-1, 3, 4).astype(np.float64), f["poses"].reshape(-1, 3, 4).astype(np.float64)
+    tr = np.einsum("nij,nij->n", Tm[:, :, :3], Tf[:, :, :3])            # trace(Rm^T Rf): the two contractions take the same LM path
+    er = np.arccos(np.clip((tr - 1.0) / 2.0, -1.0, 1.0))
+    et = np.linalg.norm(Tm[:, :, 3] - Tf[:, :, 3], axis=1)
+    assert er.max() <= 5e-3 and et.max() <= 5e-3, (er.max(), et.max())
+
+
+def test_tensor_core_path_needs_32_byte_alignment_else_falls_back():
+    """64 and more channels are gathered with 32-byte loads; a map or reference array that is only 16-byte aligned (all
+    the ABI asks for) must take the FFMA2 path instead - bit-identical to asking for FP32."""
+    import torch
+    from paper_2606_31098_b200 import binding
+    prob = tiny(seed=43, N=500, C=64, n_hyp=3, dtype="bf16", W=64, H=48)
+    P = dict(iters=[2], loss="cauchy", loss_scale=0.5, min_valid=4)
+    want = binding.refine(prob, P, mode=MODE["mode"], cluster=MODE["cluster"], math="fp32")
+    di = binding.DeviceInputs(prob)
+    feat = di.keep[0]                                       # level-0 map: the first tensor DeviceInputs uploads
+    assert feat.data_ptr() == di.inp.query_feat_dev[0] and feat.data_ptr() % 32 == 0
+    shifted = torch.empty(feat.numel() + 16, dtype=torch.uint8, device=feat.device)
+    shifted[16:].copy_(feat.view(torch.uint8).reshape(-1))
+    assert (shifted.data_ptr() + 16) % 32 == 16
+    di.inp.query_feat_dev[0] = shifted.data_ptr() + 16
+    r = binding.Refiner.for_inputs(di, P)
+    r.set_exec_mode(MODE["mode"], MODE["cluster"])
+    r.set_math_mode("mma")
+    out = r.run(di, P)
+    torch.cuda.synchronize()
+    for k in ("poses", "cost", "iter_hessian", "iter_gradient"):
+        assert np.array_equal(out[k].cpu().numpy(), want[k]), k
+    r.close()
