@@ -355,7 +355,7 @@ template <int G> struct RedRows {
 //
 // One mma covers 16 rows = (units of the round) x (32-channel slices of a pixel) x {e0, e1 | e2, e3}: thread (g, q) of
 // the fragment layout (g = lane / 4, q = lane % 4) supplies rows g and g + 8 for the channels of its 16-byte load, so
-// g = (unit, sel, slice): sel 0 loads f00, f10, f01 -> rows e0 | e2; sel 1 loads f01, f11, ref -> rows e1 | e3. The four
+// g = (sel, unit, slice): sel 0 loads f00, f10, f01 -> rows e0 | e2; sel 1 loads f01, f11, ref -> rows e1 | e3. The four
 // q-threads x two slices of a pixel read one full 128-byte line per load instruction (C = 64), as the fp32 path does.
 // B is the same registers (the Gram is symmetric): mma #1 multiplies by rows 0-7 (e0, e1), mma #2 by rows 8-15 (e2, e3);
 // only the 4 x 4 diagonal blocks (same unit, same slice) are used.
@@ -450,9 +450,11 @@ __device__ __forceinline__ void mma_unit_scalars(const float* red, int lane, flo
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
-      E[4 * i + j] = Geo::KH == 1 ? F[(i & 1) * 8 + (j >> 1) * 4 + (i >> 1) * 2 + (j & 1)]
-                                  : F[(i & 1) * 8 + (j & 1) * 4 + (j >> 1) * 2 + (i >> 1)];
+    for (int j = 0; j < 4; ++j) {                                         // E is symmetric: the block (sel 1, sel' 0) is never read
+      const int a = i <= j ? i : j, b = i <= j ? j : i;
+      const int lo = (a & 1) * 8 + (b & 1) * 4 + (b >> 1) * 2 + (a >> 1), up = (b & 1) * 8 + (a & 1) * 4 + (a >> 1) * 2 + (b >> 1);
+      E[4 * i + j] = F[((a & 1) == 1 && (b & 1) == 0) ? up : lo];
+    }
   const float ob = 1.f - b, m20 = a * ob, m21 = a * b, m22 = b - 1.f;
   float t0[2], t1[3], t2[4];                                              // t_k = E m_k (the rows that are needed)
 #pragma unroll
@@ -517,12 +519,16 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const unsigned pose_s = (unsigned)__cvta_generic_to_shared(Rc);         // Rc[9] | Cc[3] contiguous, 16-byte aligned
   const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
 
-  // fragment roles: g = (uu, sel, slice), slice in the low bits: the 8 lanes of a quarter-warp (one phase of a 16-byte
-  // load) cover one contiguous 128-byte line (C >= 64) - with sel below the slice every phase touches two lines
-  // (measured: 15.5 ms instead of 12.7 on config 4). Round r works on the units u0 + r (the owner's lane is an
-  // immediate of the shuffle).
+  // fragment roles: g = (sel, uu, slice) with sel the HIGH bit. (a) The 8 lanes of a quarter-warp (one phase of a
+  // 16-byte load) then differ in the slice bit only and cover one contiguous 128-byte line (C >= 64; with sel below the
+  // slice every phase touched two lines: 15.5 ms instead of 12.7 on config 4; a 32-byte load is one line per 4 lanes
+  // anyway). (b) Column n = 2q + c of the fragments is row-group n, and it belongs to the same (unit, slice) as row-group
+  // g iff (n & 3) == (g & 3), i.e. c = g & 1 and (q & 1) == ((g >> 1) & 1), with sel' = q >> 1: every quarter-warp has
+  // four such lanes, so the hand-off below is ONE 16-byte store per lane and round (with sel in the low bit the useful
+  // lanes were two per quarter-warp and needed two stores: 2 instead of 1 L1 wavefront per unit).
+  // Round r works on the units u0 + r.
   const int q = lane & 3, g = lane >> 2;
-  const int kap = g & (Geo::KH - 1), sel = (g >> Geo::LOGKH) & 1, uu = g >> (1 + Geo::LOGKH);
+  const int sel = g >> 2, kap = g & (Geo::KH - 1), uu = (g & 3) >> Geo::LOGKH;
   const int u0 = uu * ROUNDS;
   const unsigned tofs = (unsigned)(kap * Geo::SLICE + q * Geo::LB);
 #ifdef PILOT_PROBE_NODUP   /* tuning experiment (wrong arithmetic): sel 1 reads other lines than sel 0's f01 */
@@ -533,10 +539,9 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
 #endif
   float* const srow = red + u0 * Geo::kStride + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
-  bool useful; int js = 0;
-  if constexpr (Geo::KH == 1) useful = q == uu;
-  else { useful = Geo::KH == 2 ? (q >> 1) == uu : (q & 1) == (kap >> 1); js = Geo::KH == 2 ? (q & 1) : (q >> 1); }
-  const bool odd = kap & 1;
+  const bool useful = (q & 1) == ((g >> 1) & 1);
+  const int js = q >> 1;                                                  // sel' of this thread's useful column
+  const bool odd = g & 1;                                                 // which of its two columns that is
 
   struct Unit { float a, b, X, Y, iz, w; unsigned off; bool valid; };
   auto load_anchor = [&](int base) { const int j = base + lane; return j < end ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
@@ -584,7 +589,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
     const unsigned jmaxPX = (unsigned)min(31, L.N - 1 - base) * (unsigned)PX;
     const unsigned u0PX = (unsigned)(u0 * PX);
     auto fetch = [&](int r) {
-      const unsigned o = __shfl_sync(0xffffffffu, cur.off, r, ROUNDS);    // lane u0 + r
+      const unsigned o = __shfl_sync(0xffffffffu, cur.off, u0 + r);       // the unit's owner lane
       const unsigned o2 = sel ? min(u0PX + (unsigned)(r * PX), jmaxPX) : o;
       Raw t;
       t.l0 = ldg_words<NW>(pA + o);
@@ -615,17 +620,10 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
         M::mma(c1, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eA[2 * s], eA[2 * s + 1]);
         M::mma(c2, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eB[2 * s], eB[2 * s + 1]);
       }
-      // The 4 x 4 diagonal blocks. Column n = 2q + c of the fragments is row-group n = (uu', sel', slice').
-      float4* row = reinterpret_cast<float4*>(srow + r * Geo::kStride);
-      if constexpr (Geo::KH == 1) {                                       // n = (uu' = q, sel' = c): one thread has both columns
-        if (useful) {    // c1 = E[sel][0], E[sel][1], E[2+sel][0], E[2+sel][1];  c2 = the same rows, columns 2 and 3
-          row[0] = make_float4(c1[0], c1[1], c1[2], c1[3]);
-          row[1] = make_float4(c2[0], c2[1], c2[2], c2[3]);
-        }
-      } else {                                                            // slice' = c (KH 2) or 2 (q & 1) + c (KH 4)
-        if (useful)      // E[sel][js], E[2+sel][js], E[sel][2+js], E[2+sel][2+js]
-          row[js] = make_float4(odd ? c1[1] : c1[0], odd ? c1[3] : c1[2], odd ? c2[1] : c2[0], odd ? c2[3] : c2[2]);
-      }
+      // the 4 x 4 diagonal block of (unit u0 + r, slice kap): E[sel][js], E[2+sel][js], E[sel][2+js], E[2+sel][2+js]
+      if (useful)
+        reinterpret_cast<float4*>(srow + r * Geo::kStride)[js] =
+            make_float4(odd ? c1[1] : c1[0], odd ? c1[3] : c1[2], odd ? c2[1] : c2[0], odd ? c2[3] : c2[2]);
     }
     __syncwarp();
     float p[6];
