@@ -413,7 +413,12 @@ template <int CH> struct MmaGeom {            // CH = channels of a 16-bit featu
   static constexpr int PX = CH * 2;                    // bytes per pixel
   static constexpr int kStride = 16 * KH + 4;          // floats per unit row of the warp's buffer: [KH][4][4] + pad (odd
                                                        // multiple of 4 words: the lanes' LDS.128 are conflict-free)
-  static constexpr int kWarpFloats = 32 * kStride;
+  static constexpr int kSkew = KH == 1 ? 8 : 0;         // floats added per block of ROUNDS rows: with one slice per pixel the
+                                                       // two units that a quarter-warp hands off in a round are ROUNDS rows
+                                                       // apart (8 * 20 floats = 0 mod 32 banks); the skew moves the second one
+                                                       // 8 banks on, the lanes of a read phase share one block (no effect)
+  static constexpr int kWarpFloats = 32 * kStride + 3 * kSkew;
+  __host__ __device__ static constexpr int row(int u) { return u * kStride + kSkew * (u / ROUNDS); }
 };
 template <int G> __host__ __device__ constexpr bool mma_supported() { return G == 2 || G == 4 || G == 8 || G == 16; }
 
@@ -438,7 +443,7 @@ template <int NW> __device__ __forceinline__ TapWords<NW> ldg_words(const char* 
 template <int CH>
 __device__ __forceinline__ void mma_unit_scalars(const float* red, int lane, float a, float b, float (&p)[6]) {
   using Geo = MmaGeom<CH>;
-  const float4* rp = reinterpret_cast<const float4*>(red + lane * Geo::kStride);
+  const float4* rp = reinterpret_cast<const float4*>(red + Geo::row(lane));
   float F[16], E[16];                                                     // F: the order the fragments were stored in
 #pragma unroll
   for (int i = 0; i < 4; ++i) { const float4 t = rp[i]; F[4 * i] = t.x; F[4 * i + 1] = t.y; F[4 * i + 2] = t.z; F[4 * i + 3] = t.w; }
@@ -538,7 +543,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const char* pA = feat + tofs + (sel ? row_stride : 0u);                 // + offset: f00 | f01;  + PX: f10 | f11
   const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
 #endif
-  float* const srow = red + u0 * Geo::kStride + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
+  float* const srow = red + Geo::row(u0) + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
   const bool useful = (q & 1) == ((g >> 1) & 1);
   const int js = q >> 1;                                                  // sel' of this thread's useful column
   const bool odd = g & 1;                                                 // which of its two columns that is
