@@ -24,13 +24,13 @@ UNIT = "point-hyp-iters/s"
 LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", "iter_cost", "iter_lambda")
 
 # dram__bytes_read.sum + dram__bytes_write.sum per photo_pass_kernel launch from the committed `ncu --set full`
-# capture of this command (profiles/r1e_photo_config4.md; r1d for --math fp32: the same 34-37 MB); None where no
+# capture of this command (profiles/r1g_photo_config4.md; r1d for --math fp32: the same 34-37 MB); None where no
 # capture of that workload exists.
 NCU_TRAFFIC_BYTES = {"config4": 35.5e6}
 # From the same captures, per (anchor, hypothesis) unit-evaluation of the pass kernel at C = 64 bf16: warp instructions
 # and L1 data-pipe wavefronts (l1tex__data_pipe_lsu_wavefronts: global + shared + local + shuffles). C = 32: the
 # cluster-resident kernel (profiles/r1c_resident_small_workloads.md).
-NCU_PER_UNIT = {("mma", 64): {"inst": 29.2, "l1_wavefronts": 12.2, "source": "profiles/r1e_photo_config4.md"},
+NCU_PER_UNIT = {("mma", 64): {"inst": 30.5, "l1_wavefronts": 10.4, "source": "profiles/r1g_photo_config4.md"},
                 ("fp32", 64): {"inst": 47.5, "l1_wavefronts": 11.4, "source": "profiles/r1d_photo_config4.md"},
                 ("fp32", 32): {"inst": 32.7, "l1_wavefronts": None, "source": "profiles/r1c_resident_small_workloads.md"}}
 
@@ -515,11 +515,12 @@ def main():
                        "note": "fp32 FMA lanes: 2*(19*C+120) algorithmic flop per unit-evaluation against "
                                "SMs*128*2*1.965 GHz. With the FFMA2 contraction the kernel is issue/FMA-pipe bound "
                                "(profiles/r1d_photo_config4.md); with the tensor-core contraction the 19*C part runs as "
-                               "mma.sync and the L1 data pipe binds instead (roofline.l1)"}
+                               "mma.sync; the L1 data pipe is then the busiest unit (roofline.l1, 75 % under ncu) and the stall "
+                               "samples sit on the tap loads (profiles/r1g_photo_config4.md)"}
     per_unit = NCU_PER_UNIT.get((contraction, W.prob["channels"][-1])) if W.prob["dtype"] != "f32" else None
     units_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2))
     if per_unit and per_unit["l1_wavefronts"]:
-        # the unit that binds (profiles/r1e_photo_config4.md): the LSU data pipe moves one 128-byte wavefront per
+        # the busiest unit (profiles/r1g_photo_config4.md): the LSU data pipe moves one 128-byte wavefront per
         # clock per SM; wavefronts per unit come from the committed ncu capture, the time from this run
         l1_peak = prop.multi_processor_count * 1.965e9
         l1_rate = units_per_launch * per_unit["l1_wavefronts"] / launch_s
