@@ -537,6 +537,14 @@ def main():
     compulsory = float(map_bytes) / max(1, W.prob["n_levels"])          # one level's map read once per pass
     model = {"t_hbm_compulsory_ms": compulsory / (peak * 1e9) * 1e3, "t_fma_ms": flops_per_launch / (alu_peak * 1e12) * 1e3,
              "t_l2_gather_ms": None, "t_run_ms": launch_s * 1e3}
+    if contraction == "mma":
+        # the 19*C part is not on the FMA lanes: what stays there is the lift (2*120 flop per unit); the Gram runs as
+        # C/16 k-steps x 2 HMMA.16816 per 4 units (4096 flop each, a quarter of it useful) against the mma.sync rate
+        # measured on this pool's B200 (550 TFLOP/s dense-equivalent)
+        C_last = W.prob["channels"][-1]
+        model["t_fma_ms"] = units_per_launch * 2 * 120 / (alu_peak * 1e12) * 1e3
+        model["t_tensor_ms"] = units_per_launch * (C_last / 16.0) * 2 * 4096 / 4 / 550e12 * 1e3
+        model["fma_note"] = "mma contraction: t_fma_ms = lift only (2*120 flop per unit); t_tensor_ms = issued mma.sync flop / 550 TFLOP/s"
     if per_unit:
         model["t_issue_ms"] = units_per_launch * per_unit["inst"] / (prop.multi_processor_count * 4 * 1.965e9) * 1e3
         model["issue_source"] = "warp instructions per unit from " + per_unit["source"]
