@@ -3,8 +3,9 @@
  *
  * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT. Only tests/, __graft_entry__.smoke()
  * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
- * It shares no code with paper_2606_31098_b200/csrc (only the POD structs of
- * include/pilot_refine.h, with every "_dev" pointer holding a HOST pointer here).
+ * It shares no code and no header with the product (include/, paper_2606_31098_b200/csrc):
+ * the data interface is restated in pilot_oracle_types.h, with every "_dev" pointer
+ * holding a HOST pointer here.
  *
  * It follows the paper's algorithm step by step (arxiv/paper_2606_31098, PAPER.md):
  *   Eq.(1)-(2) photo residual / robust cost
@@ -25,7 +26,7 @@
 #ifndef PILOT_ORACLE_H
 #define PILOT_ORACLE_H
 
-#include "../include/pilot_refine.h"
+#include "pilot_oracle_types.h"
 
 #ifdef __cplusplus
 extern "C" {

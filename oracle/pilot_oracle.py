@@ -2,7 +2,7 @@
 
 TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 --impl reference legs may import this module. It imports nothing from the product package.
-All arrays are numpy host arrays. Struct layouts mirror include/pilot_refine.h.
+All arrays are numpy host arrays. Struct layouts mirror oracle/pilot_oracle_types.h (the oracle's own statement of the data interface).
 """
 import ctypes as C
 import os
@@ -68,7 +68,7 @@ class Extra(C.Structure):
 def build(force=False):
     """Compile libpilot_oracle.so with gcc (building the checker is not using it)."""
     src = os.path.join(_HERE, "pilot_oracle.c")
-    hdrs = [os.path.join(_HERE, "pilot_oracle.h"), os.path.join(_HERE, "..", "include", "pilot_refine.h")]
+    hdrs = [os.path.join(_HERE, "pilot_oracle.h"), os.path.join(_HERE, "pilot_oracle_types.h")]
     if not force and os.path.exists(_LIB):
         t = os.path.getmtime(_LIB)
         if all(os.path.getmtime(f) <= t for f in [src] + hdrs):

@@ -47,3 +47,24 @@ def test_binding_refuses_without_gpu():
     from tests.small_problems import tiny
     with pytest.raises(RuntimeError):
         binding.refine(tiny())
+
+
+def _data_interface(path):
+    """Constants, enums and POD structs of a header as a normalised token string (comments and layout removed)."""
+    src = open(path).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    items = re.findall(r"typedef\s+enum\s*\{[^}]*\}\s*\w+\s*;|typedef\s+struct\s*\{[^}]*\}\s*\w+\s*;|#define[ \t]+PILOT_\w+[ \t]+\S+", src)
+    return {re.search(r"(\w+)\s*;?$|#define\s+(\w+)", it).group(0).strip(" ;"): re.sub(r"\s+", " ", it).strip() for it in items}
+
+
+def test_oracle_types_describe_the_same_bytes_as_the_abi_header():
+    # The oracle shares no header with the product: oracle/pilot_oracle_types.h restates the data interface. Every
+    # struct, enum and constant it declares must read token for token as include/pilot_refine.h declares it.
+    abi = _data_interface(os.path.join(ROOT, "include", "pilot_refine.h"))
+    orc = _data_interface(os.path.join(ROOT, "oracle", "pilot_oracle_types.h"))
+    for name in ("pilot_refine_config", "pilot_refine_inputs", "pilot_refine_params", "pilot_refine_outputs",
+                 "pilot_dtype", "pilot_loss", "pilot_range_mode", "pilot_lm_mode", "pilot_damp_mode", "pilot_grad_mode"):
+        assert name in orc and name in abi, name
+    for name, text in orc.items():
+        assert abi.get(name) == text, name
+    assert "pilot_refine.h" not in re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "oracle", "pilot_oracle.h")).read(), flags=re.S)
