@@ -369,6 +369,26 @@ int pilot_refine_lift_anchors(const float* corners_dev, int crop_width, int crop
                               float* points_dev, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Unrolled reprojection supervision, forward value (supp III-C). For every pose
+ * T^k of poses_dev[n_poses][12] (row-major [R_wc | C], e.g. the poses of successive pilot_refine_run_levels calls) and the
+ * ground-truth pose pose_star[12] (HOST values):
+ *   L_k = 1/|V| sum_{j in V} rho_B(||pi(K, T^k P_j) - pi(K, T* P_j)||^2)                    supp Eq.(7)-(8)
+ * with Barron's general robust loss on the squared residual s, z = s/scale^2:
+ *   rho_B = |alpha-2|/alpha ((z/|alpha-2| + 1)^(alpha/2) - 1);  alpha = 2: z/2;  alpha = 0: log(z/2 + 1);
+ *   alpha = -inf: 1 - exp(-z/2).  (alpha and scale are parameters: the paper states neither.)
+ * V = points of points_dev[n_points][4] (x, y, z, unused; 16-byte aligned) in front of BOTH cameras (Z > z_near) whose
+ * ground-truth projection lies inside [0, width-1] x [0, height-1]; the optimised projection may leave the image.
+ * loss_dev[n_poses] (0 where V is empty), n_visible_dev[n_poses] = |V| (may be NULL). Projections, the loss and the
+ * sums are double precision, summed in a fixed order. Asynchronous on cuda_stream, no allocation. The backward pass
+ * through the unrolled LM steps is not part of this library.
+ * Errors: PILOT_ERR_ARG (NULL / misaligned pointer, scale <= 0, alpha NaN or +inf, bad image size), PILOT_ERR_CUDA.
+ */
+int pilot_refine_reprojection_loss(const float* poses_dev, int n_poses, const float pose_star[12],
+                                   const float* points_dev, int n_points, const float intrinsics[4],
+                                   int width, int height, float z_near, float alpha, float scale,
+                                   float* loss_dev, int* n_visible_dev, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Measurement helper: random-gather bandwidth of this GPU with the photo kernel's access
  * shape — aligned reads of vec_bytes (16..512, power of two; vec_bytes/16 lanes x 16-byte ld.global.nc) at
  * hashed positions of a buffer of buffer_bytes (e.g. 16 MiB = L2-resident, 1 GiB = HBM). Allocates and frees

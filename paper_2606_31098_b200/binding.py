@@ -33,7 +33,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
            "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
-           "pilot_refine_footprint", "pilot_refine_lift_anchors"]
+           "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
 
@@ -159,6 +159,10 @@ def lib():
         L.pilot_refine_lift_anchors.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int,
                                                 C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
         L.pilot_refine_lift_anchors.restype = C.c_int
+        L.pilot_refine_reprojection_loss.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_float), C.c_void_p, C.c_int,
+                                                     C.POINTER(C.c_float), C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
+                                                     C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_reprojection_loss.restype = C.c_int
         L.pilot_refine_probe_gather.argtypes = [C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.pilot_refine_probe_gather.restype = C.c_int
         for name in EXPORTS:
@@ -674,3 +678,23 @@ def lift_anchors(corners, crop_w, crop_h, pix, dsm, dsm_origin, dsm_gsd, stream=
                                            float(dsm_origin[1]), float(dsm_gsd), out.data_ptr(),
                                            _stream_ptr(torch, stream, pix.device)), "pilot_refine_lift_anchors")
     return out
+
+
+# ------------------------------------------------------------------ unrolled reprojection supervision (supp III-C)
+
+def reprojection_loss(poses, pose_star, points, intrinsics, width, height, z_near, alpha, scale, stream=None):
+    """supp Eq.(7)-(8), forward value. poses: cuda float32 [n, 12]; pose_star: 12 host floats; points: cuda float32
+    [N, 4]. -> (loss cuda float32 [n], n_visible cuda int32 [n])."""
+    torch = _torch()
+    assert poses.is_cuda and points.is_cuda and poses.dtype == points.dtype == torch.float32
+    assert poses.is_contiguous() and points.is_contiguous()
+    n = int(poses.shape[0])
+    K = (C.c_float * 4)(*[float(k) for k in intrinsics])
+    Ts = (C.c_float * 12)(*[float(t) for t in pose_star])
+    loss = torch.empty(n, dtype=torch.float32, device=poses.device)
+    nvis = torch.empty(n, dtype=torch.int32, device=poses.device)
+    _check(lib().pilot_refine_reprojection_loss(poses.data_ptr(), n, Ts, points.data_ptr(), int(points.shape[0]), K,
+                                                int(width), int(height), float(z_near), float(alpha), float(scale),
+                                                loss.data_ptr(), nvis.data_ptr(), _stream_ptr(torch, stream, poses.device)),
+           "pilot_refine_reprojection_loss")
+    return loss, nvis
