@@ -24,7 +24,7 @@ UNIT = "point-hyp-iters/s"
 LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", "iter_cost", "iter_lambda")
 
 # dram__bytes_read.sum + dram__bytes_write.sum per photo_pass_kernel launch from the committed `ncu --set full`
-# capture of this command (profiles/r1g_photo_config4.md; r1d for --math fp32: the same 34-37 MB); None where no
+# capture of this command (profiles/r1h_photo_config4.md, r1g before the 1536-anchor chunks; r1d for --math fp32: the same 34-37 MB); None where no
 # capture of that workload exists.
 NCU_TRAFFIC_BYTES = {"config4": 35.5e6, "config2": 18.0e6}    # config 2: profiles/r1g_photo_config2.md
 # From the same captures, per (anchor, hypothesis) unit-evaluation of the pass kernel at C = 64 bf16: warp instructions
