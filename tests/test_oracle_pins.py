@@ -6,7 +6,7 @@ CPU only (-m "not gpu").
 """
 import numpy as np
 import pytest
-from scipy.linalg import expm
+from scipy.linalg import expm, logm
 from scipy.spatial.transform import Rotation
 
 from oracle import pilot_oracle as po
@@ -527,3 +527,173 @@ def test_half_types_decode_exactly(dtype):
     R, Cv = RC(pf)
     e16, e32 = po.evaluate(po.Bound(pf), 0, R, Cv), po.evaluate(po.Bound(p32), 0, R, Cv)
     assert np.array_equal(e16["H"], e32["H"]) and np.array_equal(e16["g"], e32["g"]) and e16["cost"] == e32["cost"]
+
+
+# ------------------------------------------------------------------ round-2 pins ("What's weak" #1 a-d)
+
+def _points_at_pixels(prob, uv, depth=60.0):
+    """Anchors that project exactly (up to fp32 rounding of their coordinates) to the given pixels: the pinhole
+    back-projection written out here, independent of the oracle."""
+    fx, fy, cx, cy = prob["K"]
+    T = prob["gt_pose"].reshape(3, 4)
+    P = []
+    for u, v in uv:
+        ray = np.array([(u - cx) / fx, (v - cy) / fy, 1.0]) * depth
+        P.append(np.concatenate([T[:, 3] + T[:, :3] @ ray, [1.0]]))
+    return np.asarray(P, np.float32)
+
+
+def test_query_confidence_is_bilinear_sample_times_reference_weight():
+    """Reading A5: w = w_ref(j) * bilinear(query_conf)(u, v). A confidence map that is affine in
+    (x, y) is reproduced exactly by bilinear sampling, so w = w_ref (c0 + c1 u + c2 v) with (u, v) from the independent
+    projection written in this test. Fails if the sample drops a tap, swaps a and b, or indexes [x][y]."""
+    prob = tiny(seed=31, N=40, C=3, conf=True)
+    W, H = 40, 30
+    c0, c1, c2 = 0.31, 0.0123, -0.0071                       # asymmetric in x and y on purpose
+    ys, xs = np.mgrid[0:H, 0:W].astype(np.float64)
+    prob["query_conf"] = [(c0 + c1 * xs + c2 * ys).astype(np.float32)]
+    fx, fy, cx, cy = prob["K"]
+    T = prob["gt_pose"].reshape(3, 4)
+    R, Cv = po.pose_to_RC(T)
+    b = po.Bound(prob)
+    seen = 0
+    for j in range(40):
+        P = prob["points"][0][j].astype(np.float64)
+        pc = T[:, :3].T @ (P[:3] - T[:, 3])
+        u, v = fx * pc[0] / pc[2] + cx, fy * pc[1] / pc[2] + cy
+        o = po.photo_point(b, 0, R, Cv, j)
+        if o is None:
+            continue
+        seen += 1
+        assert P[3] != 1.0
+        assert o["w"] == pytest.approx(P[3] * (c0 + c1 * u + c2 * v), rel=2e-7, abs=1e-7)   # fp32 rounding of the map
+    assert seen >= 15
+    # and the weight enters the system as omega = w rho'(w s): with L2, H and g of one anchor scale linearly in w
+    prob1 = tiny(seed=31, N=1, C=3, conf=True)
+    prob1["points"][0][0] = prob["points"][0][7]
+    prob1["ref_feat"] = [prob["ref_feat"][0][7:8]]
+    prob1["query_conf"] = prob["query_conf"]
+    pw = dict(prob1); pw["query_conf"] = [None]; pw["points"] = [prob1["points"][0].copy()]; pw["points"][0][0, 3] = 1.0
+    e1, e0 = po.evaluate(po.Bound(prob1, dict(loss="l2")), 0, R, Cv), po.evaluate(po.Bound(pw, dict(loss="l2")), 0, R, Cv)
+    w7 = po.photo_point(po.Bound(prob1), 0, R, Cv, 0)["w"]
+    assert e1["n_valid"] == 1 and np.allclose(e1["H"], w7 * e0["H"], rtol=1e-12) and np.allclose(e1["g"], w7 * e0["g"], rtol=1e-12)
+
+
+def _T_cw(pose12):
+    T = np.asarray(pose12, np.float64).reshape(3, 4)
+    M = np.eye(4)
+    M[:3, :3] = T[:, :3].T
+    M[:3, 3] = -T[:, :3].T @ T[:, 3]
+    return M
+
+
+def _pose_of(T_cw):
+    R_wc = T_cw[:3, :3].T
+    return np.concatenate([R_wc, (-R_wc @ T_cw[:3, 3])[:, None]], 1)
+
+
+@pytest.mark.parametrize("damp", ["identity", "diag"])
+def test_lm_step_is_damped_normal_equation_and_left_retraction(damp):
+    """Eq.(8)-(9): for every recorded iteration of a small run, dxi = -(H_k + lambda_k D)^-1 g_k with
+    D = I (DAMP_IDENTITY) or diag(max(H_ii, 1e-12)) (DAMP_DIAG, reading A12), solved here with numpy from the recorded
+    system, and T_cw <- expm(dxi^) T_cw with scipy's matrix exponential. The candidate is accepted iff its total cost
+    (po.evaluate, pinned separately) is lower (LM_ADAPTIVE); the next recorded pose is the candidate if accepted, the
+    same pose if not. Fails on a doubled or missing damping term, a wrong sign of the step, right- instead of
+    left-multiplication, or an inverted accept test."""
+    prob = tiny(seed=33, N=60, C=4, n_hyp=3)
+    # lambda comparable with the Hessian's diagonal so that the damping term moves the step visibly
+    lam0 = {"identity": 30.0, "diag": 0.7}[damp]
+    prob["params"] = dict(iters=[7], loss="huber", loss_scale=0.4, min_valid=4, lambda_init=lam0, damp_mode=damp,
+                          lambda_down=0.5, lambda_up=3.0, w_gravity=0.5, gravity_scale=0.0)
+    b = po.Bound(prob)
+    o = po.run(b)
+    n_acc = n_rej = n_sharp = 0
+    prng = np.random.default_rng(5)
+    for m in range(3):
+        for k in range(7):
+            Hk = o["iter_hessian"][k, m].astype(np.float64).reshape(6, 6)
+            gk = o["iter_gradient"][k, m].astype(np.float64)
+            lam = float(o["iter_lambda"][k, m])
+            D = np.eye(6) if damp == "identity" else np.diag(np.maximum(np.diag(Hk), 1e-12))
+            A = Hk + lam * D
+            dxi = np.linalg.solve(A, -gk)                                  # library routine
+            # H, g, lambda are recorded in fp32: the sensitivity of the recomputed step to that rounding, measured by
+            # perturbing the recorded system by fp32 epsilons (a per-component tolerance, x4)
+            dev = np.zeros(6)
+            for _ in range(16):
+                Hp = Hk * (1 + 6e-8 * prng.uniform(-1, 1, (6, 6))); Hp = 0.5 * (Hp + Hp.T)
+                dev = np.maximum(dev, np.abs(np.linalg.solve(Hp + lam * (1 + 6e-8) * (np.eye(6) if damp == "identity" else np.diag(np.maximum(np.diag(Hp), 1e-12))),
+                                                             -gk * (1 + 6e-8 * prng.uniform(-1, 1, 6))) - dxi))
+            tol = 4 * dev + 1e-9
+            doubled = np.linalg.solve(Hk + 2 * lam * D, -gk)
+            sharp = np.any(np.abs(dxi - doubled) > 20 * tol)               # a doubled damping term would be caught here
+            n_sharp += sharp
+            pose_k = o["iter_poses"][k, m]
+            cand = _pose_of(expm(xi_mat(dxi)) @ _T_cw(pose_k))             # Eq.(9) on T_cw (reading A1)
+            c_cand = po.evaluate(b, 0, *po.pose_to_RC(cand))["cost"]
+            c_k = po.evaluate(b, 0, *po.pose_to_RC(pose_k))["cost"]
+            assert c_k == pytest.approx(float(o["iter_cost"][k, m]), rel=1e-6)
+            accept = c_cand < c_k
+            nxt = o["iter_poses"][k + 1, m] if k + 1 < 7 else o["poses64"][m]
+            if accept:     # compare in the twist domain: the step the oracle took is log(T_next T_k^-1)
+                Lg = np.real(logm(_T_cw(nxt) @ np.linalg.inv(_T_cw(pose_k))))
+                took = np.array([Lg[0, 3], Lg[1, 3], Lg[2, 3], Lg[2, 1], Lg[0, 2], Lg[1, 0]])
+                assert np.allclose(took, dxi, rtol=0, atol=tol), (m, k, took, dxi)
+                assert np.allclose(nxt, cand.reshape(-1), rtol=0, atol=1e-5)      # gross check; the twist comparison above is the sharp one
+            else:
+                assert np.array_equal(nxt, pose_k), (m, k)
+            if k + 1 < 7:
+                lam_next = float(o["iter_lambda"][k + 1, m])
+                assert lam_next == pytest.approx(max(lam * 0.5, 1e-8) if accept else min(lam * 3.0, 1e8), rel=1e-6)
+            n_acc += accept
+            n_rej += not accept
+    assert n_acc >= 6 and n_sharp >= 6 and n_rej == 0
+    # the reject branch: run on past convergence with the default schedule (x0.1 / x10); a step that does not lower the
+    # cost leaves the pose untouched and raises lambda, and the candidate really was no better
+    prob["params"] = dict(prob["params"], iters=[16], lambda_down=0.1, lambda_up=10.0)
+    b = po.Bound(prob)
+    o = po.run(b)
+    n_rej = 0
+    for m in range(3):
+        c, lam = o["iter_cost"][:, m], o["iter_lambda"][:, m]
+        for k in range(15):
+            same = np.array_equal(o["iter_poses"][k + 1, m], o["iter_poses"][k, m])
+            if c[k + 1] < c[k]:
+                assert not same and lam[k + 1] == pytest.approx(max(lam[k] * 0.1, 1e-8), rel=1e-6)
+                continue
+            n_rej += 1
+            assert same and c[k + 1] == c[k] and lam[k + 1] == pytest.approx(min(lam[k] * 10.0, 1e8), rel=1e-6)
+            Hk, gk = o["iter_hessian"][k, m].astype(np.float64).reshape(6, 6), o["iter_gradient"][k, m].astype(np.float64)
+            D = np.eye(6) if damp == "identity" else np.diag(np.maximum(np.diag(Hk), 1e-12))
+            cand = _pose_of(expm(xi_mat(np.linalg.solve(Hk + float(lam[k]) * D, -gk))) @ _T_cw(o["iter_poses"][k, m]))
+            c_k = po.evaluate(b, 0, *po.pose_to_RC(o["iter_poses"][k, m]))["cost"]
+            assert po.evaluate(b, 0, *po.pose_to_RC(cand))["cost"] >= c_k * (1 - 1e-9)
+    assert n_rej >= 3
+
+
+def test_central_difference_replicate_border():
+    """Reading A7: Dx[y][x] = 0.5 (F[y][min(x+1, W-1)] - F[y][max(x-1, 0)]) (replicate border), Dy likewise. On a field
+    F = s x the interior gradient is s and columns 0 and W-1 give s/2, so the bilinear sample of Dx in the border cells
+    is s (1 + a) / 2 at x0 = 0 and s (1 - a / 2) at x0 = W - 2; the same in y with F = t y. Fails if the clamp is
+    missing (reads a neighbouring row), mirrors instead of replicating, or halves the wrong column."""
+    W, H = 40, 30
+    s, t = 0.07, -0.04
+    ys, xs = np.mgrid[0:H, 0:W].astype(np.float64)
+    prob = tiny(seed=35, N=8, C=2)
+    prob["query_feat"] = [np.stack([s * xs, t * ys], -1).astype(np.float32)]
+    uv = [(0.25, 11.5), (0.8, 3.25), (W - 2 + 0.3, 17.75), (W - 2 + 0.9, 9.5),      # left / right border cells
+          (13.5, 0.4), (22.25, 0.85), (7.75, H - 2 + 0.2), (31.5, H - 2 + 0.65)]    # top / bottom border cells
+    prob["points"] = [_points_at_pixels(prob, uv)]
+    prob["ref_feat"] = [np.zeros((8, 2), np.float32)]
+    b = po.Bound(prob, dict(grad_mode="central_sampled"))
+    R, Cv = po.pose_to_RC(prob["gt_pose"])
+    for j, (u, v) in enumerate(uv):
+        o = po.photo_point(b, 0, R, Cv, j)
+        assert o is not None
+        assert np.allclose(o["uv"], [u, v], atol=2e-4)                              # fp32 anchor coordinates
+        a, bb = o["uv"][0] - np.floor(o["uv"][0]), o["uv"][1] - np.floor(o["uv"][1])
+        x0, y0 = int(np.floor(o["uv"][0])), int(np.floor(o["uv"][1]))
+        gx_want = s * (1 + a) / 2 if x0 == 0 else (s * (1 - a / 2) if x0 == W - 2 else s)
+        gy_want = t * (1 + bb) / 2 if y0 == 0 else (t * (1 - bb / 2) if y0 == H - 2 else t)
+        assert o["gx"][0] == pytest.approx(gx_want, abs=2e-7) and o["gx"][1] == pytest.approx(0.0, abs=2e-7)
+        assert o["gy"][1] == pytest.approx(gy_want, abs=2e-7) and o["gy"][0] == pytest.approx(0.0, abs=2e-7)
