@@ -39,7 +39,7 @@ extern "C" {
 #define PILOT_OK               0
 #define PILOT_ERR_ARG         (-1)  /* NULL / out-of-range argument                          */
 #define PILOT_ERR_WORKSPACE   (-2)  /* caller-provided workspace too small                   */
-#define PILOT_ERR_UNSUPPORTED (-3)  /* shape not supported (C*sizeof not pow2 multiple of 16 B, over capacity) */
+#define PILOT_ERR_UNSUPPORTED (-3)  /* shape not supported (C*sizeof not pow2 multiple of 16 B, a level map of 4 GiB or more, over capacity) */
 #define PILOT_ERR_CUDA        (-4)  /* a CUDA runtime call failed                            */
 
 /* per-hypothesis status bits (outputs.status_dev) */

@@ -178,15 +178,6 @@ struct RawTaps { uint4 q00, q10, q01, q11, ref; };
 template <int PX>   // PX = bytes per pixel = 16*G: the x+1 taps are an immediate offset away
 __device__ __forceinline__ RawTaps load_taps(const char* feat, unsigned off, unsigned row_stride, const char* ref) {
   RawTaps t;
-#ifdef PILOT_PROBE_NO_LOADS
-  { const unsigned z = off >> 31, y = row_stride >> 31;     // zero, but not to the compiler
-    t.q00 = make_uint4(0x3f803f80u | z, 0x3f003f00u | y, 0x3e803f80u | z, 0x3f803e80u | y);
-    t.q10 = make_uint4(0x3f813f80u | y, 0x3f013f00u | z, 0x3e813f80u | y, 0x3f813e80u | z);
-    t.q01 = make_uint4(0x3f823f80u | z, 0x3f023f00u | z, 0x3e823f80u | y, 0x3f823e80u | y);
-    t.q11 = make_uint4(0x3f833f80u | y, 0x3f033f00u | y, 0x3e833f80u | z, 0x3f833e80u | z);
-    t.ref = make_uint4(0x3f843f80u | z, 0x3f043f00u | y, 0x3e843f80u | y, 0x3f843e80u | z); }
-  return t;
-#endif
   const char* p = feat + off;
   const char* q = p + row_stride;
   t.q00 = ldg16(p);
@@ -220,11 +211,6 @@ template <> __device__ __forceinline__ void unpack2<F16Tag>(const uint4& v, floa
 
 template <class T>
 __device__ __forceinline__ void unit_partials(const RawTaps& t, float a, float b, float (&p)[6]) {
-#ifdef PILOT_PROBE_LOADS_ONLY   /* tuning experiment: how fast is the gather alone (loads kept alive by an XOR fold) */
-  const unsigned x = t.q00.x ^ t.q10.y ^ t.q01.z ^ t.q11.w ^ t.ref.x ^ t.q00.w ^ t.q10.z ^ t.q01.y ^ t.q11.x ^ t.ref.y;
-  p[0] = (float)(x & 0x3ffu) * 1e-6f * a; p[1] = p[2] = p[3] = p[4] = 0.f; p[5] = b;
-  return;
-#endif
   constexpr int V2 = T::kVec / 2;
   float2 f00[V2], f10[V2], f01[V2], f11[V2], fr[V2];
   unpack2<T>(t.q00, f00); unpack2<T>(t.q10, f10); unpack2<T>(t.q01, f01); unpack2<T>(t.q11, f11);
@@ -536,13 +522,8 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const int sel = g >> 2, kap = g & (Geo::KH - 1), uu = (g & 3) >> Geo::LOGKH;
   const int u0 = uu * ROUNDS;
   const unsigned tofs = (unsigned)(kap * Geo::SLICE + q * Geo::LB);
-#ifdef PILOT_PROBE_NODUP   /* tuning experiment (wrong arithmetic): sel 1 reads other lines than sel 0's f01 */
-  const char* pA = feat + tofs + (sel ? row_stride - 4u * PX : 0u);
-  const char* pF = feat + tofs + row_stride;
-#else
   const char* pA = feat + tofs + (sel ? row_stride : 0u);                 // + offset: f00 | f01;  + PX: f10 | f11
   const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
-#endif
   float* const srow = red + Geo::row(u0) + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
   const bool useful = (q & 1) == ((g >> 1) & 1);
   const int js = q >> 1;                                                  // sel' of this thread's useful column
@@ -588,6 +569,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   for (; base < end; base += step) {
 #if !PILOT_MMA_XBATCH
     const Unit cur = project(load_anchor(base), base);
+    if (!__any_sync(0xffffffffu, cur.valid)) continue;                    // no visible unit in this batch: nothing to gather
 #endif
     // the batch's reference rows are contiguous; a batch that runs over the end of the anchors clamps its rows
     const char* const p2 = sel ? refb + (size_t)base * PX + tofs : pF;     // + offset: ref | f01
@@ -763,6 +745,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
     int x0 = valid ? (int)x0d : 0, y0 = valid ? (int)y0d : 0;
     unsigned off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * px_stride;   // invalid units read pixel (0,0)
     unsigned offv = valid ? off : 0xffffffffu;
+    if (!__any_sync(0xffffffffu, valid)) continue;         // no visible unit in this batch: nothing to gather
 
     // ---- group rounds: gather + per-unit contraction (a3-a5), reduce-scatter so that lane i ends
     //      up with the six sums of unit i of this batch
@@ -849,12 +832,7 @@ __device__ __forceinline__ void photo_accumulate(const PassArgs& A, const double
     }
 
     // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
-#ifdef PILOT_PROBE_NO_LIFT
-    if (valid) { PILOT_ACC(27) += cur[0] + cur[5]; PILOT_ACC(28) += 1.f; }
-    if (false) {
-#else
     if (valid) {
-#endif
       float wq = 1.f;
       if (L.conf) {
         const float* q = L.conf + (size_t)y0 * L.W + x0;
@@ -1027,7 +1005,6 @@ __device__ bool range_prior(const PassArgs& A, const double* R, const double* C,
   J[4] = m[2] * q[0] - m[0] * q[2];
   J[5] = m[0] * q[1] - m[1] * q[0];
   if (A.prm.range_mode == PILOT_RANGE_MARCH) {
-#pragma unroll
     const double indw = fast_rcp(ndw);
 #pragma unroll
     for (int i = 0; i < 6; ++i) J[i] = -J[i] * indw;

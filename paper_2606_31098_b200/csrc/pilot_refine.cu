@@ -111,6 +111,18 @@ bool config_ok(const pilot_refine_config* c) {
   return true;
 }
 
+// Tap addresses are 32-bit byte offsets into a level's map and n_valid is summed in fp32 (exact to 2^24): larger shapes
+// are refused at create() instead of wrapping silently.
+bool shape_supported(const pilot_refine_config* c) {
+  if (c->max_points > (1 << 24)) return false;
+  for (int l = 0; l < c->n_levels; ++l) {
+    const unsigned long long bytes = (unsigned long long)c->width[l] * (unsigned long long)c->height[l] *
+                                     (unsigned long long)c->channels[l] * (unsigned long long)elem_size(c->feat_dtype);
+    if (bytes >= 0xffffffffull) return false;
+  }
+  return true;
+}
+
 struct WsLayout { size_t state, counters, partials, total; int max_chunks; };
 
 WsLayout ws_layout(const pilot_refine_config* c) {
@@ -216,6 +228,7 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   if (!config_ok(cfg)) return PILOT_ERR_ARG;
   for (int l = 0; l < cfg->n_levels; ++l)
     if (lanes_per_unit(cfg->channels[l], cfg->feat_dtype) == 0) return PILOT_ERR_UNSUPPORTED;
+  if (!shape_supported(cfg)) return PILOT_ERR_UNSUPPORTED;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return PILOT_ERR_CUDA;
   int prev = 0;

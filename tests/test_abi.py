@@ -36,6 +36,15 @@ def test_pure_host_entry_points():
     h = ctypes.c_void_p()
     assert L.pilot_refine_create(None, ctypes.byref(h)) == -1
     assert L.pilot_refine_run(None, None, None, None, None) == -1
+    # tap addresses are 32-bit byte offsets: a level map of 4 GiB or more is refused (before any CUDA call), not wrapped
+    big = binding.Config()
+    big.n_levels, big.feat_dtype = 1, 1
+    big.width[0], big.height[0], big.channels[0] = 8192, 4096, 64           # 4 GiB of bf16
+    big.max_hypotheses, big.max_points, big.max_total_iters = 4, 1024, 4
+    assert L.pilot_refine_create(ctypes.byref(big), ctypes.byref(h)) == -3 and not h.value
+    big.width[0] = 8191
+    big.max_points = (1 << 24) + 1                                          # n_valid is summed in fp32
+    assert L.pilot_refine_create(ctypes.byref(big), ctypes.byref(h)) == -3 and not h.value
 
 
 def test_binding_refuses_without_gpu():
