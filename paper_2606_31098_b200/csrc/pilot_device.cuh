@@ -163,6 +163,23 @@ __device__ __forceinline__ void robust(int loss, T x, T scale, T& rho, T& drho) 
   }
 }
 
+// The same for the 16-bit feature path, whose tolerance (5e-3) leaves room for the hardware approximations: rsqrt / rcp /
+// lg2 (MUFU, ~2^-22 relative) instead of the divide, sqrt and log1p sequences. log(1 + q) through lg2 loses RELATIVE
+// accuracy for tiny q (6e-8 / q), but its ABSOLUTE error per unit is <= 6e-8 s^2, nothing against a cost of ~N s^2.
+__device__ __forceinline__ void robust_fast(int loss, float x, float scale, float& rho, float& drho) {
+  rho = x; drho = 1.f;
+  if (scale > 0.f) {
+    const float s2 = scale * scale;
+    if (loss == PILOT_LOSS_HUBER) {
+      if (x > s2) { const float y = rsqrtf(x); rho = 2.f * scale * (x * y) - s2; drho = scale * y; }
+    } else if (loss == PILOT_LOSS_CAUCHY) {
+      const float q1 = 1.f + x * __frcp_rn(s2);
+      rho = s2 * 0.69314718056f * __log2f(q1);
+      drho = __frcp_rn(q1);
+    }
+  }
+}
+
 }  // namespace
 
 namespace {
@@ -331,7 +348,7 @@ template <int G> struct RedRows {
 //
 // For 16-bit features the C x 3 contraction of a unit (a3-a5) is a 4 x 4 Gram matrix E = D D^T of FIRST DIFFERENCES
 //   e0 = f10 - f00,  e1 = f11 - f01,  e2 = f01 - f00,  e3 = ref - f01          (rows of D, C channels each)
-// followed by three quadratic forms in the bilinear weights (mma_unit_scalars below):
+// followed by three quadratic forms in the bilinear weights (gram_unit_scalars below):
 //   gx = (1-b) e0 + b e1,   gy = -a e0 + a e1 + e2,   r = f - ref = a(1-b) e0 + ab e1 + (b-1) e2 - e3.
 // The differences are taken in the storage type (packed HSUB2: exact whenever the two values are within a factor of two
 // of each other - Sterbenz - which is every channel of a smooth map except at zero crossings; otherwise one rounding of
@@ -339,12 +356,14 @@ template <int G> struct RedRows {
 // fp32 on the tensor cores (mma.sync.m16n8k16 = HMMA.16816.F32). Differencing first is what makes the Gram safe: a
 // Gram of the raw taps would cancel by ~3e4.
 //
-// One mma covers 16 rows = (units of the round) x (32-channel slices of a pixel) x {e0, e1 | e2, e3}: thread (g, q) of
-// the fragment layout (g = lane / 4, q = lane % 4) supplies rows g and g + 8 for the channels of its 16-byte load, so
-// g = (sel, unit, slice): sel 0 loads f00, f10, f01 -> rows e0 | e2; sel 1 loads f01, f11, ref -> rows e1 | e3. The four
-// q-threads x two slices of a pixel read one full 128-byte line per load instruction (C = 64), as the fp32 path does.
-// B is the same registers (the Gram is symmetric): mma #1 multiplies by rows 0-7 (e0, e1), mma #2 by rows 8-15 (e2, e3);
-// only the 4 x 4 diagonal blocks (same unit, same slice) are used.
+// Fragment roles (round 2): ONE UNIT PER ROW-GROUP. Thread (g, q) of the fragment layout (g = lane / 4, q = lane % 4)
+// loads, for the unit of row-group g, its quarter of the pixel (C/2 bytes: one 32-byte LDG.256 at C = 64) of ALL FIVE
+// vectors - the four q-threads of a row-group read one whole pixel per instruction, 8 units = 8 lines per warp-wide load,
+// and no vector is fetched twice (round 1 split a unit over two row-groups, which cost a second fetch of f01 and a
+// 16-float hand-off per unit). It forms the four differences for its channels and issues, per 16-channel k-step,
+//   A = {e0 | e2} (rows g | g+8) x B = e0, e1, e3, e2      and      A' = {e1 | e3} x B = e1, e3
+// (B column g = the same thread's registers): the diagonal entries C[g][g], C[g+8][g] of the six accumulators are the
+// ten distinct entries of E for unit g (two come twice), and they all land in ONE thread, (g, q = g / 2).
 template <class T> struct MmaType;
 template <> struct MmaType<BF16Tag> {
   static __device__ __forceinline__ unsigned sub2(unsigned x, unsigned y) {
@@ -355,6 +374,10 @@ template <> struct MmaType<BF16Tag> {
   static __device__ __forceinline__ void mma(float (&c)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
     asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+  }
+  static __device__ __forceinline__ void mma0(float (&c)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+        : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(0.f));
   }
 };
 template <> struct MmaType<F16Tag> {
@@ -367,85 +390,52 @@ template <> struct MmaType<F16Tag> {
     asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
   }
+  static __device__ __forceinline__ void mma0(float (&c)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+        : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(0.f));
+  }
 };
 template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features stay on the FFMA2 path
 
-#ifndef PILOT_MMA_XBATCH
-#define PILOT_MMA_XBATCH 0      // 1: anchors and projection of the NEXT batch overlap the first taps of the current one
-                                // (config 4 at 128 registers, prefetch 6: 12.57 ms without, 11.27 ms with; no room at 64)
-#endif
-#ifndef PILOT_MMA_SHFL_ACC
-#define PILOT_MMA_SHFL_ACC 1      // 1: per-batch shuffle reduce-scatter into ONE accumulator register per lane (no
-                                  // shared-memory columns, no 29 live registers): what lets the kernel run at 64 registers
-#endif
-#ifndef PILOT_MMA_PREFETCH_REGS
-#define PILOT_MMA_PREFETCH_REGS 24   // registers of taps in flight ahead of the tensor-core arithmetic: 1 round of 32-byte
-                                     // loads, 2 rounds of 16-byte loads (one round = three loads per thread)
-#endif
-#ifndef PILOT_MMA_LB32
-#define PILOT_MMA_LB32 1        // 1: 64 and more channels use 32-byte loads (LDG.256): half the load instructions and rounds
-#endif
-
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
-  static constexpr int LBMAX = PILOT_MMA_LB32 ? 32 : 16;
-  static constexpr int LB = CH / 2 < LBMAX ? CH / 2 : LBMAX;   // bytes per load per thread (the 4 q-threads share a slice)
-  static constexpr int NW = LB / 4;                    // 32-bit words (= pairs of channels) per load per thread
-  static constexpr int KS = NW / 2;                    // k-steps of 16 channels per mma chain
-  static constexpr int SLICE = 4 * LB;                 // bytes of a pixel that one row-group covers
-  static constexpr int KH = 2 * CH / SLICE;            // slices per pixel
-  static constexpr int LOGKH = KH == 4 ? 2 : (KH == 2 ? 1 : 0);
-  static constexpr int UR = 4 / KH;                    // units per round
-  static constexpr int ROUNDS = 32 / UR;
   static constexpr int PX = CH * 2;                    // bytes per pixel
-  static constexpr int kStride = 16 * KH + 4;          // floats per unit row of the warp's buffer: [KH][4][4] + pad (odd
-                                                       // multiple of 4 words: the lanes' LDS.128 are conflict-free)
-  static constexpr int kSkew = KH == 1 ? 8 : 0;         // floats added per block of ROUNDS rows: with one slice per pixel the
-                                                       // two units that a quarter-warp hands off in a round are ROUNDS rows
-                                                       // apart (8 * 20 floats = 0 mod 32 banks); the skew moves the second one
-                                                       // 8 banks on, the lanes of a read phase share one block (no effect)
-  static constexpr int kWarpFloats = 32 * kStride + 3 * kSkew;
-  __host__ __device__ static constexpr int row(int u) { return u * kStride + kSkew * (u / ROUNDS); }
+  static constexpr int TB = PX / 4 < 32 ? PX / 4 : 32; // bytes per load per thread (the 4 q-threads share a pixel): 8, 16, 32
+  static constexpr int NW = TB / 4;                    // 32-bit words (= pairs of channels) per load per thread
+  static constexpr int KS = NW / 2;                    // k-steps of 16 channels per load
+  static constexpr int PARTS = PX / (4 * TB);          // loads per vector per thread (2 at 128 channels)
+  static constexpr int LB = TB;                        // (alignment the loads need: 32 bytes from 64 channels on)
+  static constexpr int kRow = 12;                      // floats per unit row of the warp's hand-off buffer: the ten distinct
+                                                       // entries of E + 2 pad; 8 consecutive rows x 16 B fall in 8 distinct
+                                                       // groups of four banks (12 i mod 32 = 0,12,24,4,16,28,8,20)
+  static constexpr int kSlotFloats = 64;               // 32 x {tap offset, anchor index in the batch}
+  static constexpr int kWarpFloats = kSlotFloats + 32 * kRow;
 };
 template <int G> __host__ __device__ constexpr bool mma_supported() { return G == 2 || G == 4 || G == 8 || G == 16; }
 
 template <int NW> struct TapWords { unsigned w[NW]; };
+#ifndef PILOT_LDG_OP
+#define PILOT_LDG_OP "ld.global.nc"
+#endif
 template <int NW> __device__ __forceinline__ TapWords<NW> ldg_words(const char* p) {
   TapWords<NW> t;
   if constexpr (NW == 8) {                     // 32-byte load (sm_100: LDG.256); p is 32-byte aligned
-    asm("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+    asm volatile(PILOT_LDG_OP ".v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
         : "=r"(t.w[0]), "=r"(t.w[1]), "=r"(t.w[2]), "=r"(t.w[3]), "=r"(t.w[4]), "=r"(t.w[5]), "=r"(t.w[6]), "=r"(t.w[7]) : "l"(p));
   } else if constexpr (NW == 4) {
-    const uint4 v = ldg16(p);
-    t.w[0] = v.x; t.w[1] = v.y; t.w[2] = v.z; t.w[3] = v.w;
+    asm volatile(PILOT_LDG_OP ".v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(t.w[0]), "=r"(t.w[1]), "=r"(t.w[2]), "=r"(t.w[3]) : "l"(p));
   } else {
-    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p));
-    t.w[0] = v.x; t.w[1] = v.y;
+    asm volatile(PILOT_LDG_OP ".v2.b32 {%0,%1}, [%2];" : "=r"(t.w[0]), "=r"(t.w[1]) : "l"(p));
   }
   return t;
 }
 
-// Lane phase: lane i reads the Gram matrix of unit i (summing the 32-channel slices in a fixed order) and forms
+// Lane phase: the unit's lane reads the ten distinct entries of its Gram matrix E (row = three float4:
+// {E00, E01, E02, E03}, {E11, E12, E13, E22}, {E23, E33, -, -}) and forms
 //   p = { gx.gx, gx.gy, gy.gy, gx.r, gy.r, r.r } = M E M^T, M = rows of the three combinations above.
-template <int CH>
-__device__ __forceinline__ void mma_unit_scalars(const float* red, int lane, float a, float b, float (&p)[6]) {
-  using Geo = MmaGeom<CH>;
-  const float4* rp = reinterpret_cast<const float4*>(red + Geo::row(lane));
-  float F[16], E[16];                                                     // F: the order the fragments were stored in
-#pragma unroll
-  for (int i = 0; i < 4; ++i) { const float4 t = rp[i]; F[4 * i] = t.x; F[4 * i + 1] = t.y; F[4 * i + 2] = t.z; F[4 * i + 3] = t.w; }
-#pragma unroll
-  for (int k = 1; k < Geo::KH; ++k) {
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { const float4 t = rp[4 * k + i]; F[4 * i] += t.x; F[4 * i + 1] += t.y; F[4 * i + 2] += t.z; F[4 * i + 3] += t.w; }
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {                                         // E is symmetric: the block (sel 1, sel' 0) is never read
-      const int a = i <= j ? i : j, b = i <= j ? j : i;
-      const int lo = (a & 1) * 8 + (b & 1) * 4 + (b >> 1) * 2 + (a >> 1), up = (b & 1) * 8 + (a & 1) * 4 + (a >> 1) * 2 + (b >> 1);
-      E[4 * i + j] = F[((a & 1) == 1 && (b & 1) == 0) ? up : lo];
-    }
+__device__ __forceinline__ void gram_unit_scalars(const float* row, float a, float b, float (&p)[6]) {
+  const float4 r0 = reinterpret_cast<const float4*>(row)[0], r1 = reinterpret_cast<const float4*>(row)[1];
+  const float2 r2 = reinterpret_cast<const float2*>(row)[4];
+  const float E[16] = {r0.x, r0.y, r0.z, r0.w,  r0.y, r1.x, r1.y, r1.z,  r0.z, r1.y, r1.w, r2.x,  r0.w, r1.z, r2.x, r2.y};
   const float ob = 1.f - b, m20 = a * ob, m21 = a * b, m22 = b - 1.f;
   float t0[2], t1[3], t2[4];                                              // t_k = E m_k (the rows that are needed)
 #pragma unroll
@@ -464,7 +454,7 @@ __device__ __forceinline__ void mma_unit_scalars(const float* red, int lane, flo
 
 // floats of the [kNacc][kThreads] accumulator array in dynamic shared memory (0: accumulators in registers)
 template <bool MMA> __host__ __device__ constexpr int acc_smem_floats() {
-  return (MMA && PILOT_MMA_SHFL_ACC) ? 0 : (PILOT_SMEM_ACC ? kNacc * kThreads : 0);
+  return MMA ? 0 : (PILOT_SMEM_ACC ? kNacc * kThreads : 0);
 }
 template <int G, bool MMA> __host__ __device__ constexpr int red_warp_floats() {
   if constexpr (MMA) return MmaGeom<8 * G>::kWarpFloats; else return RedRows<G>::kWarpFloats;
@@ -478,56 +468,41 @@ template <int G, bool MMA> constexpr size_t gather_smem_bytes() {
 
 // ------------------------------------------------------------------ the photo gather, tensor-core contraction
 //
-// Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on batches of 32 units:
-//   lane-per-unit   anchor load, projection + visibility in fp64 (a2) - done ONE BATCH AHEAD, while the first taps
-//                   of the current batch are in flight, so that the tap latency at the head of a batch is covered;
-//   fragment roles  ROUNDS rounds of (HSUB2 differences -> 2 KS mma.sync) over UR units each, taps prefetched
-//                   PILOT_MMA_PREFETCH_REGS registers ahead; the 4 x 4 diagonal blocks go to the warp's buffer `red`;
-//   lane-per-unit   Gram -> six scalars, robust weight, lift through J_uv, accumulate (a4-a6).
+// Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on batches of 32 anchors:
+//   lane-per-unit   anchor load (one batch ahead), projection + visibility in fp64 (a2); the VISIBLE units of the batch are
+//                   compacted (ballot + popc rank): their tap offset and anchor index go to slot `rank` of the warp's table,
+//                   a batch with no visible unit is skipped, and only ceil(n_visible / 8) rounds run;
+//   fragment roles  per round, row-group g takes slot 8 r + g: five loads, four packed differences per word,
+//                   6 KS mma.sync; thread (g, g / 2) hands the unit's ten Gram entries to row `slot` of the warp's buffer;
+//   lane-per-unit   the unit's own lane reads its row: Gram -> six scalars, robust weight, lift through J_uv, and the batch is
+//                   reduce-scattered over the warp into one accumulator register per lane (a4-a6).
 template <class T, int G>
 __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const double* Rc, const double* Ccand,
                                                      int begin, int end, int worker, int n_workers,
                                                      float (&acc)[kNacc], float* sacc, float* red) {
-#if PILOT_SMEM_ACC
-#define PILOT_MACC(i) sacc[(i) * kThreads]
-#else
-#define PILOT_MACC(i) acc[i]
-#endif
   constexpr int CH = 8 * G;
   using Geo = MmaGeom<CH>;
   using M = MmaType<T>;
-  constexpr int NW = Geo::NW, PX = Geo::PX, ROUNDS = Geo::ROUNDS;
-  constexpr int PFW = PILOT_MMA_PREFETCH_REGS / (3 * NW) < 1 ? 1 : PILOT_MMA_PREFETCH_REGS / (3 * NW);
-  constexpr int PF = PFW < ROUNDS ? PFW : ROUNDS;
+  constexpr int NW = Geo::NW, PX = Geo::PX, KS = Geo::KS;
   const LevelArgs& L = A.lv;
   const int lane = threadIdx.x & 31;
   const unsigned row_stride = (unsigned)PX * (unsigned)L.W;
   const char* feat = static_cast<const char*>(L.feat);
   const char* refb = static_cast<const char*>(L.ref);
 
-  // The candidate pose stays in SHARED memory (Rc[9] and Ccand = Rc + 9 must point there, 16-byte aligned) and is re-read by every projection: as 24
-  // registers held across the rounds it forced the address arithmetic of every round to be rematerialised.
+  // The candidate pose stays in SHARED memory (Rc[9] and Ccand = Rc + 9 must point there, 16-byte aligned) and is re-read
+  // by every projection: as 24 registers held across the rounds it forced the address arithmetic to be rematerialised.
   const unsigned pose_s = (unsigned)__cvta_generic_to_shared(Rc);         // Rc[9] | Cc[3] contiguous, 16-byte aligned
   const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
 
-  // fragment roles: g = (sel, uu, slice) with sel the HIGH bit. (a) The 8 lanes of a quarter-warp (one phase of a
-  // 16-byte load) then differ in the slice bit only and cover one contiguous 128-byte line (C >= 64; with sel below the
-  // slice every phase touched two lines: 15.5 ms instead of 12.7 on config 4; a 32-byte load is one line per 4 lanes
-  // anyway). (b) Column n = 2q + c of the fragments is row-group n, and it belongs to the same (unit, slice) as row-group
-  // g iff (n & 3) == (g & 3), i.e. c = g & 1 and (q & 1) == ((g >> 1) & 1), with sel' = q >> 1: every quarter-warp has
-  // four such lanes, so the hand-off below is ONE 16-byte store per lane and round (with sel in the low bit the useful
-  // lanes were two per quarter-warp and needed two stores: 2 instead of 1 L1 wavefront per unit).
-  // Round r works on the units u0 + r.
   const int q = lane & 3, g = lane >> 2;
-  const int sel = g >> 2, kap = g & (Geo::KH - 1), uu = (g & 3) >> Geo::LOGKH;
-  const int u0 = uu * ROUNDS;
-  const unsigned tofs = (unsigned)(kap * Geo::SLICE + q * Geo::LB);
-  const char* pA = feat + tofs + (sel ? row_stride : 0u);                 // + offset: f00 | f01;  + PX: f10 | f11
-  const char* pF = pA + row_stride;                                       // sel 0: + offset: f01
-  float* const srow = red + Geo::row(u0) + kap * 16 + sel * 8;       // + r * kStride: this thread's block of unit u0 + r
-  const bool useful = (q & 1) == ((g >> 1) & 1);
-  const int js = q >> 1;                                                  // sel' of this thread's useful column
-  const bool odd = g & 1;                                                 // which of its two columns that is
+  const bool diag = q == (g >> 1);                                        // holds C[g][g] and C[g+8][g] of every accumulator
+  const bool odd = g & 1;                                                 // ... in c[1], c[3] (else c[0], c[2])
+  const char* const featq = feat + q * Geo::TB;
+  const char* const refq = refb + q * Geo::TB;
+  uint2* const slots = reinterpret_cast<uint2*>(red);
+  float* const rows = red + Geo::kSlotFloats;
+  const unsigned rows_s = (unsigned)__cvta_generic_to_shared(rows);
 
   struct Unit { float a, b, X, Y, iz, w; unsigned off; bool valid; };
   auto load_anchor = [&](int base) { const int j = base + lane; return j < end ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
@@ -552,79 +527,87 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
     U.a = valid ? (float)(ud - x0d) : 0.f;
     U.b = valid ? (float)(vd - y0d) : 0.f;
     const int x0 = valid ? (int)x0d : 0, y0 = valid ? (int)y0d : 0;
-    U.off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * (unsigned)PX;   // invisible units gather pixel (0,0)
+    U.off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * (unsigned)PX;
     U.X = (float)Xd; U.Y = (float)Yd; U.iz = (float)izd; U.w = P.w; U.valid = valid;
     return U;
   };
 
-  struct Raw { TapWords<NW> l0, l1, l2; };
   const int step = n_workers * 32;
   int base = begin + worker * 32;
   if (base >= end) return;
-#if PILOT_MMA_XBATCH
   float4 Pn = load_anchor(base);
-  Unit cur = project(Pn, base);
-  Pn = load_anchor(base + step);
-#endif
   for (; base < end; base += step) {
-#if !PILOT_MMA_XBATCH
-    const Unit cur = project(load_anchor(base), base);
-    if (!__any_sync(0xffffffffu, cur.valid)) continue;                    // no visible unit in this batch: nothing to gather
-#endif
-    // the batch's reference rows are contiguous; a batch that runs over the end of the anchors clamps its rows
-    const char* const p2 = sel ? refb + (size_t)base * PX + tofs : pF;     // + offset: ref | f01
-    const unsigned jmaxPX = (unsigned)min(31, L.N - 1 - base) * (unsigned)PX;
-    const unsigned u0PX = (unsigned)(u0 * PX);
-    auto fetch = [&](int r) {
-      const unsigned o = __shfl_sync(0xffffffffu, cur.off, u0 + r);       // the unit's owner lane
-      const unsigned o2 = sel ? min(u0PX + (unsigned)(r * PX), jmaxPX) : o;
-      Raw t;
-      t.l0 = ldg_words<NW>(pA + o);
-      t.l1 = ldg_words<NW>(pA + o + PX);
-      t.l2 = ldg_words<NW>(p2 + o2);
-      return t;
-    };
-    Raw buf[PF];
-#pragma unroll
-    for (int d = 0; d < PF; ++d) buf[d] = fetch(d);
+    const Unit cur = project(Pn, base);
+    Pn = load_anchor(base + step);                                        // next batch's anchors: in flight during this batch
+    const unsigned vmask = __ballot_sync(0xffffffffu, cur.valid);
+    if (vmask == 0u) continue;                                            // no visible unit in this batch: nothing to gather
+    const int nv = __popc(vmask);
+    const int rank = __popc(vmask & ((1u << lane) - 1u));
+    if (cur.valid) slots[rank] = make_uint2(cur.off, (unsigned)(base + lane));
+    __syncwarp();
 
-#if PILOT_MMA_XBATCH
-    // next batch: projection while the first taps are in flight; its anchors were loaded one batch ago
-    const Unit nxt = project(Pn, base + step);
-    Pn = load_anchor(base + 2 * step);
-#endif
-
+    const int nr = (nv + 7) >> 3;
+    for (int r = 0; r < nr; ++r) {
+      const int s = 8 * r + g;
+      const bool act = s < nv;
+      float c0[4], c1[4], c2[4], c3[4], c4[4], c5[4];
+      // a row-group past the last visible unit repeats slot 0 (always there: its loads hit L1) and stores nothing
+      const uint2 sl = slots[act ? s : 0];
+      const char* const p0 = featq + sl.x;
+      const char* const pr = refq + (size_t)sl.y * PX;
 #pragma unroll
-    for (int r = 0; r < ROUNDS; ++r) {
-      const Raw t = buf[r % PF];
-      if (r + PF < ROUNDS) buf[r % PF] = fetch(r + PF);
-      unsigned eA[NW], eB[NW];
+      for (int part = 0; part < Geo::PARTS; ++part) {
+        const TapWords<NW> f00 = ldg_words<NW>(p0 + part * 128);
+        const TapWords<NW> f10 = ldg_words<NW>(p0 + part * 128 + PX);
+        const TapWords<NW> f01 = ldg_words<NW>(p0 + part * 128 + row_stride);
+        const TapWords<NW> f11 = ldg_words<NW>(p0 + part * 128 + row_stride + PX);
+        const TapWords<NW> fr = ldg_words<NW>(pr + part * 128);
 #pragma unroll
-      for (int i = 0; i < NW; ++i) { eA[i] = M::sub2(t.l1.w[i], t.l0.w[i]); eB[i] = M::sub2(t.l2.w[i], t.l0.w[i]); }
-      float c1[4] = {0.f, 0.f, 0.f, 0.f}, c2[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-      for (int s = 0; s < Geo::KS; ++s) {
-        M::mma(c1, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eA[2 * s], eA[2 * s + 1]);
-        M::mma(c2, eA[2 * s], eB[2 * s], eA[2 * s + 1], eB[2 * s + 1], eB[2 * s], eB[2 * s + 1]);
+        for (int k = 0; k < KS; ++k) {
+          const unsigned e0a = M::sub2(f10.w[2 * k], f00.w[2 * k]), e0b = M::sub2(f10.w[2 * k + 1], f00.w[2 * k + 1]);
+          const unsigned e1a = M::sub2(f11.w[2 * k], f01.w[2 * k]), e1b = M::sub2(f11.w[2 * k + 1], f01.w[2 * k + 1]);
+          const unsigned e2a = M::sub2(f01.w[2 * k], f00.w[2 * k]), e2b = M::sub2(f01.w[2 * k + 1], f00.w[2 * k + 1]);
+          const unsigned e3a = M::sub2(fr.w[2 * k], f01.w[2 * k]), e3b = M::sub2(fr.w[2 * k + 1], f01.w[2 * k + 1]);
+          if (part == 0 && k == 0) {
+            M::mma0(c0, e0a, e2a, e0b, e2b, e0a, e0b);                    // e0.e0 | e2.e0
+            M::mma0(c1, e0a, e2a, e0b, e2b, e1a, e1b);                    // e0.e1 | e2.e1
+            M::mma0(c2, e0a, e2a, e0b, e2b, e3a, e3b);                    // e0.e3 | e2.e3
+            M::mma0(c3, e0a, e2a, e0b, e2b, e2a, e2b);                    // (e0.e2) | e2.e2
+            M::mma0(c4, e1a, e3a, e1b, e3b, e1a, e1b);                    // e1.e1 | e3.e1
+            M::mma0(c5, e1a, e3a, e1b, e3b, e3a, e3b);                    // (e1.e3) | e3.e3
+          } else {
+            M::mma(c0, e0a, e2a, e0b, e2b, e0a, e0b);
+            M::mma(c1, e0a, e2a, e0b, e2b, e1a, e1b);
+            M::mma(c2, e0a, e2a, e0b, e2b, e3a, e3b);
+            M::mma(c3, e0a, e2a, e0b, e2b, e2a, e2b);
+            M::mma(c4, e1a, e3a, e1b, e3b, e1a, e1b);
+            M::mma(c5, e1a, e3a, e1b, e3b, e3a, e3b);
+          }
+        }
       }
-      // the 4 x 4 diagonal block of (unit u0 + r, slice kap): E[sel][js], E[2+sel][js], E[sel][2+js], E[2+sel][2+js]
-      if (useful)
-        reinterpret_cast<float4*>(srow + r * Geo::kStride)[js] =
-            make_float4(odd ? c1[1] : c1[0], odd ? c1[3] : c1[2], odd ? c2[1] : c2[0], odd ? c2[3] : c2[2]);
+      if (diag && act) {
+        const unsigned rp = rows_s + (unsigned)(s * Geo::kRow) * 4u;
+        const float E00 = odd ? c0[1] : c0[0], E02 = odd ? c0[3] : c0[2];
+        const float E01 = odd ? c1[1] : c1[0], E12 = odd ? c1[3] : c1[2];
+        const float E03 = odd ? c2[1] : c2[0], E23 = odd ? c2[3] : c2[2];
+        const float E22 = odd ? c3[3] : c3[2];
+        const float E11 = odd ? c4[1] : c4[0], E13 = odd ? c4[3] : c4[2];
+        const float E33 = odd ? c5[3] : c5[2];
+        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp), "f"(E00), "f"(E01), "f"(E02), "f"(E03) : "memory");
+        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp + 16u), "f"(E11), "f"(E12), "f"(E13), "f"(E22) : "memory");
+        asm volatile("st.shared.v2.f32 [%0], {%1,%2};" :: "r"(rp + 32u), "f"(E23), "f"(E33) : "memory");
+      }
     }
     __syncwarp();
-    float p[6];
-    mma_unit_scalars<CH>(red, lane, cur.a, cur.b, p);
-    __syncwarp();                                                         // rows are rewritten by the next batch
 
-    // ---- lane-per-unit: robust weight, lift through the 2x6 Jacobian, accumulate (a4-a6)
-#if PILOT_MMA_SHFL_ACC
+    // ---- lane-per-unit: Gram -> six scalars, robust weight, lift through the 2x6 Jacobian (a4-a6)
     float v[32];
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = 0.f;
-#endif
     if (cur.valid) {
       const float a = cur.a, b = cur.b;
+      float p[6];
+      gram_unit_scalars(rows + rank * Geo::kRow, a, b, p);
       float wq = 1.f;
       if (L.conf) {
         const float* cq = L.conf + cur.off / (unsigned)PX;
@@ -633,7 +616,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       }
       float w = cur.w * wq;
       float rho, drho;
-      robust<float>(A.prm.loss, w * p[5], A.prm.loss_scale, rho, drho);
+      robust_fast(A.prm.loss, w * p[5], A.prm.loss_scale, rho, drho);
       float om = w * drho;
       float x = cur.X * cur.iz, y = cur.Y * cur.iz;
       float fxz = L.fx * cur.iz, fyz = L.fy * cur.iz;
@@ -641,7 +624,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       float Jv[6] = {0.f, fyz, -fyz * y, -L.fy * (1.f + y * y), L.fy * x * y, L.fy * x};
       float A11 = om * p[0], A12 = om * p[1], A22 = om * p[2];
       float b1 = om * p[3], b2 = om * p[4];
-#if PILOT_MMA_SHFL_ACC
 #pragma unroll
       for (int i = 0; i < 6; ++i) {
         float mu = A11 * Ju[i] + A12 * Jv[i];
@@ -652,20 +634,8 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       }
       v[27] = rho;
       v[28] = 1.f;
-#else
-#pragma unroll
-      for (int i = 0; i < 6; ++i) {
-        float mu = A11 * Ju[i] + A12 * Jv[i];
-        float mv = A12 * Ju[i] + A22 * Jv[i];
-#pragma unroll
-        for (int k = i; k < 6; ++k) PILOT_MACC(tri(i, k)) += mu * Ju[k] + mv * Jv[k];
-        PILOT_MACC(21 + i) += b1 * Ju[i] + b2 * Jv[i];
-      }
-      PILOT_MACC(27) += rho;
-      PILOT_MACC(28) += 1.f;
-#endif
     }
-#if PILOT_MMA_SHFL_ACC
+    __syncwarp();                                                         // rows and slots are rewritten by the next batch
     // reduce-scatter of the batch over the warp: lane i ends with the batch total of component i (31 shuffles), which
     // goes to ONE accumulator register per lane: no shared-memory traffic, no 29 live registers
 #pragma unroll
@@ -679,12 +649,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       }
     }
     acc[0] += v[0];
-#endif
-#if PILOT_MMA_XBATCH
-    cur = nxt;
-#endif
   }
-#undef PILOT_MACC
 }
 
 // ------------------------------------------------------------------ the photo kernel
@@ -879,40 +844,46 @@ inline size_t gather_smem_for(int g, bool mma) {
 }
 
 // The per-thread accumulators before / after photo_accumulate: registers, a column of shared memory, or (tensor-core
-// path with PILOT_MMA_SHFL_ACC) one register per lane that already holds the warp total of component `lane`.
+// path) one register per lane that already holds the warp total of component `lane`.
 #define PILOT_DECLARE_ACC extern __shared__ float4 pilot_dyn_smem[]; \
   float* sacc = reinterpret_cast<float*>(pilot_dyn_smem) + threadIdx.x; float acc[kNacc]; \
   float* red = reinterpret_cast<float*>(pilot_dyn_smem) + acc_smem_floats<MMA>() + (threadIdx.x >> 5) * red_warp_floats<G, MMA>();
 
 template <bool MMA>
 __device__ __forceinline__ void acc_zero(float (&acc)[kNacc], float* sacc) {
-  if constexpr (MMA && PILOT_MMA_SHFL_ACC) { acc[0] = 0.f; return; }
+  if constexpr (MMA) {
+    acc[0] = 0.f;
+  } else {
 #pragma unroll
-  for (int i = 0; i < kNacc; ++i) {
-    if (PILOT_SMEM_ACC) sacc[i * kThreads] = 0.f; else acc[i] = 0.f;
+    for (int i = 0; i < kNacc; ++i) {
+      if (PILOT_SMEM_ACC) sacc[i * kThreads] = 0.f; else acc[i] = 0.f;
+    }
   }
 }
 
 // Warp total of component `lane` (fixed order: deterministic).
 template <bool MMA>
 __device__ __forceinline__ float acc_warp_total(float (&acc)[kNacc], const float* sacc, int lane) {
-  if constexpr (MMA && PILOT_MMA_SHFL_ACC) return acc[0];
-  if (PILOT_SMEM_ACC) {
+  if constexpr (MMA) {
+    return acc[0];
+  } else {
+    if (PILOT_SMEM_ACC) {
 #pragma unroll
-    for (int i = 0; i < kNacc; ++i) acc[i] = sacc[i * kThreads];
-  }
-  // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
-#pragma unroll
-  for (int half = 16; half >= 1; half >>= 1) {
-    const bool upper = lane & half;
-#pragma unroll
-    for (int i = 0; i < half; ++i) {
-      float send = upper ? acc[i] : acc[i + half];
-      float keep = upper ? acc[i + half] : acc[i];
-      acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+      for (int i = 0; i < kNacc; ++i) acc[i] = sacc[i * kThreads];
     }
+    // reduce-scatter over the warp: lane i ends with the warp total of component i (31 shuffles)
+#pragma unroll
+    for (int half = 16; half >= 1; half >>= 1) {
+      const bool upper = lane & half;
+#pragma unroll
+      for (int i = 0; i < half; ++i) {
+        float send = upper ? acc[i] : acc[i + half];
+        float keep = upper ? acc[i + half] : acc[i];
+        acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
+      }
+    }
+    return acc[0];
   }
-  return acc[0];
 }
 
 }  // namespace
@@ -1255,7 +1226,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
 
 // The same on the state in the workspace (global memory): lane 0 works on a private copy, so that the optimiser
 // state sits in registers / L1 instead of being re-read from L2 around every output store. Warp-collective.
-__device__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane) {
+__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane) {
   HypState loc;
   const HypState& g = A.state[m];
   if (lane == 0) {

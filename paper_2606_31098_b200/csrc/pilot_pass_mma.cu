@@ -7,7 +7,7 @@
 // Shares no code with oracle/.
 #ifndef PILOT_MMA_THREADS
 #define PILOT_MMA_THREADS 128
-#define PILOT_MMA_MIN_BLOCKS 7
+#define PILOT_MMA_MIN_BLOCKS 6
 #endif
 #define PILOT_THREADS PILOT_MMA_THREADS
 #define PILOT_MIN_BLOCKS PILOT_MMA_MIN_BLOCKS
