@@ -23,29 +23,12 @@ METRIC = "point-hypothesis LM iterations/sec"
 UNIT = "point-hyp-iters/s"
 LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", "iter_cost", "iter_lambda")
 
-# dram__bytes_read.sum + dram__bytes_write.sum per photo_pass_kernel launch from the committed `ncu --set full`
-# capture of this command (profiles/r1h_photo_config4.md, r1g before the 1536-anchor chunks; r1d for --math fp32: the same 34-37 MB); None where no
-# capture of that workload exists.
-NCU_TRAFFIC_BYTES = {"config4": 35.5e6, "config2": 18.0e6}    # config 2: profiles/r1g_photo_config2.md
-# From the same captures, per (anchor, hypothesis) unit-evaluation of the pass kernel at C = 64 bf16: warp instructions
-# and L1 data-pipe wavefronts (l1tex__data_pipe_lsu_wavefronts: global + shared + local + shuffles). C = 32: the
-# cluster-resident kernel (profiles/r1c_resident_small_workloads.md).
-NCU_PER_UNIT = {("mma", 64): {"inst": 30.5, "l1_wavefronts": 10.4, "source": "profiles/r1g_photo_config4.md"},
-                ("fp32", 64): {"inst": 47.5, "l1_wavefronts": 11.4, "source": "profiles/r1d_photo_config4.md"},
-                ("fp32", 32): {"inst": 32.7, "l1_wavefronts": None, "source": "profiles/r1c_resident_small_workloads.md"}}
-
-
-def contraction_used(args, prob, H):
-    """Which per-unit contraction the library takes for this run (pilot_math_mode, include/pilot_refine.h): mirrors
-    AUTO's rule so that the roofline constants match the kernel that ran."""
-    C, N = prob["channels"][-1], max(p.shape[0] for p in prob["points"])
-    applies = prob["dtype"] != "f32" and C in (16, 32, 64, 128)
-    if args.math == "fp32" or not applies:
-        return "fp32"
-    if args.math == "mma":
-        return "mma"
-    resident = args.mode == "resident" or (args.mode == "auto" and H * N <= 1500000 and H <= 296)
-    return "mma" if C >= 64 and not resident else "fp32"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from the committed `ncu --set full`
+# captures of this command (profiles/<file>): the first EVAL pass of a timed step (hypotheses spread over their initial
+# poses: the union of their footprints covers the map) and a late pass (hypotheses converged onto one pose). None where
+# no capture of that workload exists. Labelled with their source; everything else in the line is measured in this run.
+NCU_TRAFFIC = {"config4": {"first_pass_bytes": 423.1e6, "converged_pass_bytes": 31.6e6,
+                           "source": "profiles/r2_photo_config4.md"}}
 
 
 def load_peaks():
@@ -88,9 +71,18 @@ class ClockSampler(threading.Thread):
 
 # ------------------------------------------------------------------ problems
 
+SHUFFLE = {"on": False}
+
+
 def make_problem(name, rank):
     from paper_2606_31098_b200 import workloads as wl
     prob = wl.make(name)
+    if SHUFFLE["on"]:          # a caller that does not sort its anchors: same problem, random anchor order
+        rng = np.random.Generator(np.random.PCG64(wl.BASE_SEED + 77))
+        for l in range(prob["n_levels"]):
+            perm = rng.permutation(prob["points"][l].shape[0])
+            prob["points"][l] = np.ascontiguousarray(prob["points"][l][perm])
+            prob["ref_feat"][l] = np.ascontiguousarray(prob["ref_feat"][l][perm])
     if rank:  # weak scaling: every rank refines its own shard of hypotheses around the same scene
         rng = np.random.Generator(np.random.PCG64(wl.BASE_SEED + 1000 * rank))
         T = prob["gt_pose"].reshape(3, 4)
@@ -138,6 +130,15 @@ class Resident:
     @property
     def launches(self):
         return self.ref.last_launches + (1 if self.torch.distributed.is_initialized() else 0)
+
+    def visible_evals(self, stream):
+        """(visible, all) (anchor, hypothesis) unit evaluations of one step: every EVAL pass of every level."""
+        it = self.params["iters"]
+        total = sum(self.H * self.prob["points"][l].shape[0] * (it[l] + 1) for l in range(self.prob["n_levels"]))
+        return self.ref.last_visible_evals(stream), total
+
+    def plan(self):
+        return self.ref.last_plan()
 
     def check(self):
         cost = self.out["cost"].cpu().numpy()
@@ -225,6 +226,13 @@ class Streaming:
     def launches(self):
         return self.ref.last_launches + 2
 
+    def visible_evals(self, stream):
+        total = sum(self.H * self.seq.N * (k + 1) for k in self.seq.iters)
+        return self.ref.last_visible_evals(stream), total
+
+    def plan(self):
+        return self.ref.last_plan()
+
     def check(self):
         gt = self.seq.gt_pose((self.i - 1) % self.RING + 1).reshape(-1)
         err = np.linalg.norm(self.best[1].cpu().numpy().reshape(3, 4)[:, 3] - gt.reshape(3, 4)[:, 3])
@@ -296,6 +304,15 @@ class PaperSchedule:
     def launches(self):
         return self.pr.launches
 
+    def visible_evals(self, stream):
+        it = self.params["iters"]
+        self.pr.run(self.prior, stream, count_visible=True)
+        total = self.H0 * 500 * (it[0] + 1) + self.keep * 500 * ((it[1] + 1) + (it[2] + 1))
+        return sum(self.pr.visible_evals), total
+
+    def plan(self):
+        return self.pr.ref.last_plan()
+
     def check(self):
         gt = self.prob["gt_pose"].reshape(3, 4)[:, 3]
         err = np.linalg.norm(self.out["best_pose"].cpu().numpy().reshape(3, 4)[:, 3] - gt)
@@ -340,7 +357,7 @@ class PaperSchedule:
     def cpu_time(self, cores):
         from oracle import pilot_hypotheses as ph
         from oracle import pilot_oracle as po
-        from tests import parity
+        from paper_2606_31098_b200 import workloads as parity       # levels_slice: dict slicing only
         p = self.prob
         t0 = time.perf_counter()
         seeds = ph.seed_hypotheses(p["prior_pose"], self.off, ph.SEED_WORLD)
@@ -386,7 +403,7 @@ def reference_problem(name):
         return wl.with_poses(f, ph.seed_hypotheses(seq.gt_pose(0).reshape(-1), seq.offsets, ph.SEED_CAMERA))
     if name == "paper":
         from oracle import pilot_hypotheses as ph
-        from tests import parity
+        parity = wl                                                  # levels_slice: dict slicing only
         p = wl.paper_frame()
         off = ph.grid_offsets(p["grid"][0], p["grid"][1], p["grid"][2], -p["gravity_world"])
         q = parity.levels_slice(p, 0, 1, ph.seed_hypotheses(p["prior_pose"], off, ph.SEED_WORLD))
@@ -400,65 +417,37 @@ def run_reference(args, rank):
         return
     prob = reference_problem(args.config)
     cores = os.cpu_count() or 1
-    vals, desc, threads = [], "", 1
+    vals, times, desc, threads = [], [], "", 1
     for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
         v, desc, threads = oracle_sample(prob, cores, budget_hyps=max(2, min(cores, 16)))
         if i >= args.warmup:
             vals.append(v)
+            times.append(time.perf_counter() - t0)
     value = float(np.mean(vals))
     H = prob["init_poses"].shape[0]
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * prob["units"] / value, "higher_is_better": True, "scaling": "weak",
+            "ms_per_step": 1e3 * float(np.mean(times)), "ms_per_step_extrapolated_to_full_workload": 1e3 * prob["units"] / value,
+            "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.config, "hypotheses": H, "points": int(prob["points"][0].shape[0]),
-                       "note": "CPU oracle (oracle/pilot_oracle.c) on a bounded hypothesis sample per step; "
-                               "ms_per_step extrapolated to the whole workload"},
+                       "note": "CPU oracle (oracle/pilot_oracle.c); a step = a bounded hypothesis sample of the workload "
+                               "(see cpu_baseline.sample): ms_per_step is the measured time of that sample, value the "
+                               "rate, which does not depend on the sample because hypotheses are independent"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
-# ------------------------------------------------------------------ main
+# ------------------------------------------------------------------ measurement
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="config4", choices=sorted(WORKLOADS))
-    ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA of the pass kernel (0 = heuristic)")
-    ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident", "split"], help="launch strategy (pilot_exec_mode)")
-    ap.add_argument("--math", default="auto", choices=["auto", "fp32", "mma"], help="per-unit contraction (pilot_math_mode)")
-    ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-probe", action="store_true", help="skip the gather-peak micro-benchmark")
-    args = ap.parse_args()
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
-        return run_reference(args, rank)
-
+def measure(W, steps, warmup, stream, local_rank, world, use_dist, flush):
+    """W untimed warm-up steps, then `steps` timed steps (CUDA events on the launching stream, a barrier and a device
+    synchronise on both sides, max over ranks), the SM clock sampled during the timed region."""
     import torch
     import torch.distributed as dist
-    from paper_2606_31098_b200 import binding
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    use_dist = world > 1 or "RANK" in os.environ        # under torchrun (also with one rank) the NCCL path runs
-    if use_dist:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    W = WORKLOADS[args.config](args, rank, local_rank, world)
-    stream = torch.cuda.current_stream(local_rank)
-    map_bytes = W.map_bytes()
-    l2_bytes = torch.cuda.get_device_properties(local_rank).L2_cache_size
-    need_flush = map_bytes <= l2_bytes
-    flush = torch.empty(max(2 * l2_bytes, 1 << 28), dtype=torch.uint8, device=f"cuda:{local_rank}") if need_flush else None
-    warmup = max(3, args.warmup)
 
     def barrier():
         if use_dist:
@@ -468,10 +457,10 @@ def main():
     for _ in range(warmup):
         W.step(stream)
     barrier()
-    launches_per_step = W.launches
+    launches = W.launches
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier()
     for s, e in ev:
         if flush is not None:
@@ -487,121 +476,210 @@ def main():
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     total_ms = float(t.item())
-    units = W.units
-    value = world * units * args.steps / (total_ms * 1e-3)
     W.check()
+    vis, tot = W.visible_evals(stream)
+    return {"ms_per_step": total_ms / steps, "value": world * W.units * steps / (total_ms * 1e-3), "launches": launches,
+            "clocks": sampler.summary(), "visible_evals": vis, "all_evals": tot}
 
-    # ---- roofline of the dominant kernel (photo_pass_kernel): algorithmic gather bytes per launch / launch time
-    launch_s = (total_ms * 1e-3 / args.steps) / W.pass_launches   # init / seed / select kernels and gaps included: conservative
-    peak, peak_src = load_peaks()
-    achieved = W.bytes_per_launch / launch_s / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(args.config), "kernel": "photo_pass_kernel",
-                "algorithmic_bytes_per_launch": W.bytes_per_launch, "launch_ms": launch_s * 1e3,
-                "peak_source": peak_src,
-                "note": "4*C*s gather bytes per (anchor,hypothesis) unit x H*N units per launch (north_star's "
-                        "HBM-gather roofline, no-reuse model); the taps are served through L2, so achieved may "
-                        "exceed the HBM copy peak when L2 reuse is high"}
-    # the bound that actually applies: plain fp32 arithmetic. Algorithmic flops per unit-evaluation =
-    # 2*(19*C + 120); peak = SMs x 128 fp32 lanes x 2 flop x max SM clock
-    prop = torch.cuda.get_device_properties(local_rank)
-    flops_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2)) \
-        * 2 * (19 * W.prob["channels"][-1] + 120)
-    alu_peak = prop.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
-    contraction = contraction_used(args, W.prob, getattr(W, "H", None) or getattr(W, "keep", 1))
-    roofline["contraction"] = contraction
-    roofline["alu"] = {"bound": "alu", "achieved": flops_per_launch / launch_s / 1e12, "peak": alu_peak,
-                       "unit": "TFLOP/s", "frac": flops_per_launch / launch_s / 1e12 / alu_peak,
-                       "note": "fp32 FMA lanes: 2*(19*C+120) algorithmic flop per unit-evaluation against "
-                               "SMs*128*2*1.965 GHz. With the FFMA2 contraction the kernel is issue/FMA-pipe bound "
-                               "(profiles/r1d_photo_config4.md); with the tensor-core contraction the 19*C part runs as "
-                               "mma.sync; the L1 data pipe is then the busiest unit (roofline.l1, 75 % under ncu) and the stall "
-                               "samples sit on the tap loads (profiles/r1g_photo_config4.md)"}
-    per_unit = NCU_PER_UNIT.get((contraction, W.prob["channels"][-1])) if W.prob["dtype"] != "f32" else None
-    units_per_launch = W.bytes_per_launch / (4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2))
-    if per_unit and per_unit["l1_wavefronts"]:
-        # the busiest unit (profiles/r1g_photo_config4.md): the LSU data pipe moves one 128-byte wavefront per
-        # clock per SM; wavefronts per unit come from the committed ncu capture, the time from this run
-        l1_peak = prop.multi_processor_count * 1.965e9
-        l1_rate = units_per_launch * per_unit["l1_wavefronts"] / launch_s
-        roofline["l1"] = {"bound": "l1-data-pipe", "achieved": l1_rate / 1e9, "peak": l1_peak / 1e9, "unit": "Gwavefront/s",
-                          "frac": l1_rate / l1_peak, "wavefronts_per_unit": per_unit["l1_wavefronts"],
-                          "algorithmic_wavefronts_per_unit": (4 * W.prob["channels"][-1] * 2 + W.prob["channels"][-1] * 2) / 128.0,
-                          "source": per_unit["source"],
-                          "note": "l1tex__data_pipe_lsu_wavefronts per unit (global + shared + shuffles + local) x units "
-                                  "per launch / launch time against SMs x 1 wavefront/clk x 1.965 GHz; the algorithmic "
-                                  "floor is the 4 taps + the reference row (5 x 128 B at C = 64 bf16)"}
-    # t_model = max(compulsory HBM bytes / HBM peak, gather bytes / L2 gather peak, flops / FMA
-    # peak); the L2 term is filled in below when the probe runs. Instruction issue (warp instructions per unit from
-    # the committed ncu captures) is listed beside it because it is the term that binds.
+
+def roofline_of(W, m, name, peaks, hbm_peak, hbm_src, map_bytes, l2_bytes):
+    """The dominant kernel's roofline. What binds is the gather of the taps from L2 into the SMs (the
+    maps are L2-resident, or - config 4 - the union of the co-resident CTAs' footprints is: 30-420 MB of DRAM traffic per
+    pass against GBs of taps), so `bound` is "l2-gather": achieved = tap bytes of the VISIBLE units (4*C*s each, SURVEY's
+    per-unit figure; invisible units move nothing) per EVAL pass / the pass's share of the step time, peak = the same
+    access shape without arithmetic from an L2-resident buffer, measured in this run by pilot_refine_probe_unit_gather.
+    north_star's "HBM-gather roofline" (every tap byte of every unit from HBM, no reuse) is reported beside it."""
+    es = 4 if W.prob["dtype"] == "f32" else 2
+    C_last = W.prob["channels"][-1]
+    unit_bytes = 4 * C_last * es
+    passes = W.pass_launches
+    pass_s = m["ms_per_step"] * 1e-3 / passes          # seed / init / select kernels and launch gaps included: conservative
+    vis_per_pass, all_per_pass = m["visible_evals"] / passes, m["all_evals"] / passes
+    achieved = vis_per_pass * unit_bytes / pass_s / 1e9
+    achieved_all = all_per_pass * unit_bytes / pass_s / 1e9
+    pk = peaks.get(C_last * es) if peaks else None
+    mma, res = W.plan()
+    r = {"bound": "l2-gather", "achieved": achieved, "peak": pk["l2_ldg_gbs"] if pk else None, "unit": "GB/s",
+         "frac": achieved / pk["l2_ldg_gbs"] if pk and pk["l2_ldg_gbs"] else None,
+         "traffic": None, "kernel": "lm_resident_kernel (K+1 passes per launch)" if res else "photo_pass_kernel (one pass per launch)",
+         "algorithmic_bytes_per_pass": vis_per_pass * unit_bytes, "pass_ms": pass_s * 1e3, "eval_passes_per_step": passes,
+         "bytes_per_visible_unit": unit_bytes, "visible_fraction": m["visible_evals"] / max(1, m["all_evals"]),
+         "contraction": "mma.sync (tensor cores)" if mma else "FFMA2", "levels_on_tensor_cores": mma, "levels_resident": res,
+         "peak_source": "pilot_refine_probe_unit_gather: unit-shaped random gather (2x2 pixels + reference row, four lanes per "
+                        "unit) from a 16 MiB buffer, measured in this run" if pk else "probe skipped",
+         "hbm_no_reuse": {"achieved_all_units": achieved_all, "achieved_visible_units": achieved, "peak": hbm_peak, "unit": "GB/s",
+                          "frac_all_units": achieved_all / hbm_peak, "frac_visible_units": achieved / hbm_peak,
+                          "peak_source": hbm_src,
+                          "note": "north_star's HBM-gather roofline: 4*C*s bytes per unit as if every tap crossed HBM once "
+                                  "(all H*N units, SURVEY.md §8(d).1; target >= 0.60 on config 4). HBM does not bind: the "
+                                  "taps are served from L2 (see traffic), so this ratio may exceed 1"}}
+    t = NCU_TRAFFIC.get(name)
+    if t:
+        r["traffic"] = t["first_pass_bytes"]
+        r["traffic_converged_pass"] = t["converged_pass_bytes"]
+        r["traffic_source"] = t["source"] + " (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum of one launch)"
+    if pk:
+        r["gather_peaks"] = pk
     compulsory = float(map_bytes) / max(1, W.prob["n_levels"])          # one level's map read once per pass
-    model = {"t_hbm_compulsory_ms": compulsory / (peak * 1e9) * 1e3, "t_fma_ms": flops_per_launch / (alu_peak * 1e12) * 1e3,
-             "t_l2_gather_ms": None, "t_run_ms": launch_s * 1e3}
-    if contraction == "mma":
-        # the 19*C part is not on the FMA lanes: what stays there is the lift (2*120 flop per unit); the Gram runs as
-        # C/16 k-steps x 2 HMMA.16816 per 4 units (4096 flop each, a quarter of it useful) against the mma.sync rate
-        # measured on this pool's B200 (550 TFLOP/s dense-equivalent)
-        C_last = W.prob["channels"][-1]
-        model["t_fma_ms"] = units_per_launch * 2 * 120 / (alu_peak * 1e12) * 1e3
-        model["t_tensor_ms"] = units_per_launch * (C_last / 16.0) * 2 * 4096 / 4 / 550e12 * 1e3
-        model["fma_note"] = "mma contraction: t_fma_ms = lift only (2*120 flop per unit); t_tensor_ms = issued mma.sync flop / 550 TFLOP/s"
-    if per_unit:
-        model["t_issue_ms"] = units_per_launch * per_unit["inst"] / (prop.multi_processor_count * 4 * 1.965e9) * 1e3
-        model["issue_source"] = "warp instructions per unit from " + per_unit["source"]
-        if per_unit["l1_wavefronts"]:
-            model["t_l1_pipe_ms"] = units_per_launch * per_unit["l1_wavefronts"] / (prop.multi_processor_count * 1.965e9) * 1e3
-    roofline["model"] = model
-    if rank == 0 and not args.no_probe:
-        # the build's own micro-benchmark: random gathers with the kernel's access shape
-        tap = 4 * W.prob["channels"][-1] * (4 if W.prob["dtype"] == "f32" else 2) // 4      # one tap = one pixel
-        tap = 1 << (tap.bit_length() - 1)
-        l2g = binding.probe_gather(16 << 20, tap, 5, local_rank)
-        hbmg = binding.probe_gather(4 << 30, tap, 5, local_rank)
-        roofline["gather_peaks"] = {"vec_bytes": tap, "l2_resident_16MiB_gbs": l2g, "hbm_4GiB_gbs": hbmg,
-                                    "frac_of_l2_gather_peak": achieved / l2g if l2g else None,
-                                    "frac_of_hbm_gather_peak": achieved / hbmg if hbmg else None,
-                                    "source": "pilot_refine_probe_gather, measured in this run"}
-        model["t_l2_gather_ms"] = W.bytes_per_launch / (l2g * 1e9) * 1e3 if l2g else None
-    terms = {k: v for k, v in model.items() if k.startswith("t_") and k != "t_run_ms" and v}
-    model["binds"] = max(terms, key=terms.get)
-    model["t_model_over_t_run"] = max(terms.values()) / model["t_run_ms"]
+    model = {"t_hbm_compulsory_ms": compulsory / (hbm_peak * 1e9) * 1e3,
+             "t_hbm_first_pass_ms": t["first_pass_bytes"] / (hbm_peak * 1e9) * 1e3 if t else None,
+             "t_l2_gather_ms": vis_per_pass * unit_bytes / (pk["l2_ldg_gbs"] * 1e9) * 1e3 if pk and pk["l2_ldg_gbs"] else None,
+             "t_pass_ms": pass_s * 1e3}
+    terms = {k: v for k, v in model.items() if k != "t_pass_ms" and v}
+    if terms:
+        model["binds"] = max(terms, key=terms.get)
+        model["t_model_over_t_pass"] = max(terms.values()) / model["t_pass_ms"]
+    r["model"] = model
+    return r
 
-    # ---- end to end through the C-ABI with HOST buffers: H2D of every input + D2H of the outputs per step
+
+def gather_peaks(binding, px_sizes, local_rank):
+    """The build's own micro-benchmark for every pixel size the workloads use."""
+    out = {}
+    for px in sorted(set(px_sizes)):
+        if px not in (64, 128):
+            continue
+        out[px] = {"px_bytes": px,
+                   "l2_ldg_gbs": binding.probe_unit_gather(16 << 20, px, 0, 5, local_rank),
+                   "l2_staged_bulk_gbs": binding.probe_unit_gather(16 << 20, px, 1, 5, local_rank),
+                   "hbm_ldg_gbs": binding.probe_unit_gather(4 << 30, px, 0, 3, local_rank),
+                   "note": "GB/s of tap bytes (4 pixels per unit; the reference row moves too, uncounted). ldg = the kernel's "
+                           "access shape; staged_bulk = cp.async.bulk into shared memory + LDS.128 (north_star's staged "
+                           "variant, measured and not adopted: profiles/r2_staged_vs_ldg.md)"}
+    return out
+
+
+def dtype_string(W):
+    mma, _ = W.plan()
+    d = W.prob["dtype"]
+    if d == "f32":
+        return "f32"
+    return d + (" storage; first differences in %s, products on mma.sync with f32 accumulate" % d if mma else " storage, f32 FFMA2 contraction") + \
+        "; f32 lift, f64 projection and 6x6 solve"
+
+
+def run_workload(name, args, rank, local_rank, world, use_dist, stream, steps, peaks, hbm, l2_bytes, with_e2e, with_cpu):
+    import torch
+    import torch.distributed as dist
+    if name != args.config:                # one of the default run's other workloads: heuristics only
+        args = argparse.Namespace(**vars(args))
+        args.config, args.mode, args.math, args.chunk, args.cluster = name, "auto", "auto", 0, 0
+    W = WORKLOADS[name](args, rank, local_rank, world)
+    map_bytes = W.map_bytes()
+    need_flush = map_bytes <= l2_bytes
+    flush = torch.empty(max(2 * l2_bytes, 1 << 28), dtype=torch.uint8, device=f"cuda:{local_rank}") if need_flush else None
+    warmup = max(3, args.warmup)
+    m = measure(W, steps, warmup, stream, local_rank, world, use_dist, flush)
+    roof = roofline_of(W, m, name, peaks, hbm[0], hbm[1], map_bytes, l2_bytes)
     e2e = None
-    if not args.no_e2e:
-        n_e2e = max(1, min(args.steps, 10))
-        barrier()
+    if with_e2e:
+        n_e2e = max(1, min(steps, 10))
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize(local_rank)
         dt, h2d, d2h = W.e2e(stream, n_e2e)
         n_e2e = getattr(W, "e2e_steps", n_e2e)
         tt = torch.tensor([dt], dtype=torch.float64, device=f"cuda:{local_rank}")
         if world > 1:
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * units * n_e2e / float(tt.item()), "unit": UNIT,
+        e2e = {"value": world * W.units * n_e2e / float(tt.item()), "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e}
-
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if with_cpu and rank == 0 and world == 1:
         cores = os.cpu_count() or 1
         cp = W.cpu_problem()
         v, desc, threads = oracle_sample(cp, cores) if cp is not None else W.cpu_time(cores)
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+        if cp is not None:                 # the single-thread figure BASELINE.md §3 plans, on a smaller sample
+            v1, d1, _ = oracle_sample(cp, 1, budget_hyps=2)
+            cpu["value_1_core"] = v1
+            cpu["sample_1_core"] = d1
+    cfg = {"workload": name, "exec_mode": args.mode, "math_mode": args.math}
+    cfg.update(W.config())
+    cfg.update({"map_bytes": map_bytes, "l2_bytes": int(l2_bytes),
+                "l2_policy": "L2 flushed between timed steps" if need_flush else "inputs larger than L2"})
+    res = {"ms_per_step": m["ms_per_step"], "value": m["value"], "steps": steps, "warmup": warmup, "dtype": dtype_string(W),
+           "config": cfg, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(m["launches"] * steps),
+           "clocks": m["clocks"]}
+    W.close()
+    del W, flush
+    torch.cuda.empty_cache()
+    return res
+
+
+# ------------------------------------------------------------------ main
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="config4", choices=sorted(WORKLOADS))
+    ap.add_argument("--chunk", type=int, default=0, help="anchors per CTA of the pass kernel (0 = heuristic)")
+    ap.add_argument("--mode", default="auto", choices=["auto", "passes", "resident", "split"], help="launch strategy (pilot_exec_mode)")
+    ap.add_argument("--math", default="auto", choices=["auto", "fp32", "mma"], help="per-unit contraction (pilot_math_mode)")
+    ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
+    ap.add_argument("--shuffle-anchors", action="store_true", help="hand the anchors over in a random order instead of the "
+                    "generator's Morton order (config1/2/4): measures what the caller's ordering is worth")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-probe", action="store_true", help="skip the gather-peak micro-benchmark")
+    ap.add_argument("--no-others", action="store_true", help="default run only: skip the other workloads' lines")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+    SHUFFLE["on"] = args.shuffle_anchors
+
+    import torch
+    import torch.distributed as dist
+    from paper_2606_31098_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    use_dist = world > 1 or "RANK" in os.environ        # under torchrun (also with one rank) the NCCL path runs
+    if use_dist:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    stream = torch.cuda.current_stream(local_rank)
+    l2_bytes = torch.cuda.get_device_properties(local_rank).L2_cache_size
+    hbm = load_peaks()
+    default_run = args.config == "config4" and world == 1 and not args.no_others and not args.shuffle_anchors
+    peaks = None
+    if rank == 0 and not args.no_probe:
+        peaks = gather_peaks(binding, [64, 128] if default_run else [128 if args.config in ("config2", "config4") else 64], local_rank)
+    main_res = run_workload(args.config, args, rank, local_rank, world, use_dist, stream, args.steps, peaks, hbm, l2_bytes,
+                            not args.no_e2e, not args.no_cpu_baseline)
+    others = None
+    if default_run and rank == 0:
+        # the other BASELINE.json configs and the paper's own schedule, in the same process and under the same clock
+        # sampling, so that the driver's record carries all five (each is well under a second of GPU time per step)
+        others = {}
+        for name in ("config1", "config2", "config3", "paper"):
+            r = run_workload(name, args, rank, local_rank, world, use_dist, stream, min(args.steps, 10), peaks, hbm, l2_bytes,
+                             not args.no_e2e, False)
+            others[name] = {k: r[k] for k in ("ms_per_step", "value", "steps", "dtype", "e2e", "gpu_launches", "clocks")}
+            others[name]["config"] = {k: r["config"][k] for k in ("hypotheses_per_gpu", "points", "channels", "iters", "l2_policy")}
+            others[name]["roofline"] = {k: r["roofline"].get(k) for k in ("bound", "achieved", "peak", "unit", "frac", "kernel",
+                                                                          "visible_fraction", "contraction", "pass_ms")}
+            others[name]["roofline"]["hbm_no_reuse_frac_all_units"] = r["roofline"]["hbm_no_reuse"]["frac_all_units"]
 
     if rank == 0:
-        cfg = {"workload": args.config, "exec_mode": args.mode, "math_mode": args.math}
-        cfg.update(W.config())
-        cfg.update({"map_bytes": map_bytes, "l2_bytes": int(l2_bytes),
-                    "l2_policy": "L2 flushed between timed steps" if need_flush else "inputs larger than L2",
-                    "sharding": "hypotheses across ranks, no data-path collective; one 13-float-per-hypothesis "
-                                "all-gather + arg-min ends the step when n_gpus > 1"})
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None,
-                "dtype": "f32" if contraction == "fp32" else W.prob["dtype"] + " mma.sync products, f32 accumulate; f32 elsewhere",
-                "data": "synthetic", "config": cfg,
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-                "gpu_launches": int(launches_per_step * args.steps), "clocks": sampler.summary()}
+        cfg = main_res["config"]
+        cfg["sharding"] = ("hypotheses across ranks, no data-path collective; one 13-float-per-hypothesis "
+                           "all-gather + arg-min ends the step when n_gpus > 1")
+        if args.shuffle_anchors:
+            cfg["anchor_order"] = "random permutation (--shuffle-anchors)"
+        line = {"metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": main_res["warmup"], "ms_per_step": main_res["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": main_res["dtype"], "data": "synthetic", "config": cfg,
+                "roofline": main_res["roofline"], "cpu_baseline": main_res["cpu_baseline"], "e2e": main_res["e2e"],
+                "gpu_launches": main_res["gpu_launches"], "clocks": main_res["clocks"]}
+        if others is not None:
+            line["other_workloads"] = others
         print(json.dumps(line))
-    W.close()
     if use_dist:
         dist.destroy_process_group()
 

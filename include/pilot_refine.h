@@ -209,6 +209,19 @@ int pilot_refine_set_math_mode(pilot_refine_handle* h, int mode);
 /* Number of kernel launches the last pilot_refine_run on this handle enqueued (host counter). */
 int pilot_refine_last_launches(const pilot_refine_handle* h);
 
+/* What the last run (or run_levels) of this handle chose per pyramid level: bit l of *mma_levels = the tensor-core
+ * contraction (pilot_math_mode), bit l of *resident_levels = the cluster-resident kernel (pilot_exec_mode). Pure host
+ * call; either pointer may be NULL. bench.py reports these instead of mirroring the AUTO rules.
+ */
+int pilot_refine_last_plan(const pilot_refine_handle* h, unsigned* mma_levels, unsigned* resident_levels);
+
+/* Measurement helper: the number of VISIBLE (anchor, hypothesis) unit evaluations of the handle's last run, summed over
+ * every EVAL pass of every level (a unit is visible iff Z > z_near and its 2 x 2 footprint lies inside the map: a2 of
+ * SURVEY.md §8(a), "visibility checking" PAPER.md:485) - the units that actually gather taps; bench.py's roofline counts
+ * bytes for these only. Runs one tiny kernel on cuda_stream and SYNCHRONISES that stream. out_host: host pointer.
+ */
+int pilot_refine_last_visible_evals(pilot_refine_handle* h, void* cuda_stream, unsigned long long* out_host);
+
 /*
  * The same as pilot_refine_run restricted to pyramid levels level_begin <= l < level_end
  * (0 <= level_begin < level_end <= n_levels): what the paper's schedule needs to prune the
@@ -396,6 +409,21 @@ int pilot_refine_reprojection_loss(const float* poses_dev, int n_poses, const fl
  * the best GB/s. Not part of the refinement path.
  */
 int pilot_refine_probe_gather(int device, size_t buffer_bytes, int vec_bytes, int launches, double* gbps_out);
+
+/* The same for the access shape of one (anchor, hypothesis) unit of the tensor-core gather (kernel description PAPER.md:485,
+ * "descriptor interpolation"): a warp reads rounds of 8 random units, each 2 x 2 pixels of px_bytes (64 or
+ * 128: 32 or 64 bf16 channels) - the two x-adjacent pixels contiguous, the two map rows 1920 pixels apart - plus one
+ * reference row of px_bytes, from a buffer of buffer_bytes (16 MiB = L2-resident: the denominator of bench.py's binding
+ * roofline; 4 GiB = HBM). variant 0: the product's shape, four lanes per unit with one px_bytes/4-byte ld.global.nc each
+ * per vector (LDG.256 at 128 bytes), 6, 8 and 12 resident CTAs of 4 warps per SM, the best taken. variant 1: the same bytes
+ * staged through shared memory with cp.async.bulk (three bulk copies per unit issued by lanes 0-7, mbarrier completion,
+ * three rounds in flight per warp) and read back with LDS.128 - north_star's "staged via TMA or shared memory" variant,
+ * kept as a measurement so that the choice is a number (profiles/r2_staged_vs_ldg.md). Writes the best GB/s of TAP bytes
+ * (4 * px_bytes per unit; the reference row is moved as well and not counted, as in SURVEY.md §8(d)'s 4*C*s per unit).
+ * Allocates and frees its own buffer, times `launches` launches with CUDA events on the default stream and SYNCHRONISES.
+ * PILOT_ERR_ARG for other px_bytes / variants or a buffer under 65536 pixels. Not part of the refinement path.
+ */
+int pilot_refine_probe_unit_gather(int device, size_t buffer_bytes, int px_bytes, int variant, int launches, double* gbps_out);
 
 #ifdef __cplusplus
 }

@@ -33,6 +33,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sequence_create", "pilot_refine_sequence_set_prior", "pilot_refine_sequence_upload",
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
            "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
+           "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
            "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
@@ -165,6 +166,12 @@ def lib():
         L.pilot_refine_reprojection_loss.restype = C.c_int
         L.pilot_refine_probe_gather.argtypes = [C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.pilot_refine_probe_gather.restype = C.c_int
+        L.pilot_refine_probe_unit_gather.argtypes = [C.c_int, C.c_size_t, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.pilot_refine_probe_unit_gather.restype = C.c_int
+        L.pilot_refine_last_visible_evals.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_ulonglong)]
+        L.pilot_refine_last_visible_evals.restype = C.c_int
+        L.pilot_refine_last_plan.argtypes = [C.c_void_p, C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
+        L.pilot_refine_last_plan.restype = C.c_int
         for name in EXPORTS:
             if name.startswith("pilot_refine_sequence_"):
                 getattr(L, name).restype = C.c_int
@@ -376,6 +383,22 @@ class Refiner:
     @property
     def last_launches(self):
         return lib().pilot_refine_last_launches(self.handle)
+
+    def last_plan(self):
+        """(mma_levels, resident_levels) bit masks of the last run: which levels used the tensor-core contraction / the
+        cluster-resident kernel."""
+        a, b = C.c_uint(), C.c_uint()
+        _check(lib().pilot_refine_last_plan(self.handle, C.byref(a), C.byref(b)), "pilot_refine_last_plan")
+        return int(a.value), int(b.value)
+
+    def last_visible_evals(self, stream=None):
+        """Visible (anchor, hypothesis) unit evaluations of the last run, all passes and levels (synchronises the stream)."""
+        if stream is None:
+            stream = self.torch.cuda.current_stream(self.device)
+        n = C.c_ulonglong()
+        _check(lib().pilot_refine_last_visible_evals(self.handle, C.c_void_p(stream.cuda_stream), C.byref(n)),
+               "pilot_refine_last_visible_evals")
+        return int(n.value)
 
     def close(self):
         if self.handle:
@@ -622,20 +645,25 @@ class PrunedRefiner:
         def __init__(self, di, inp, n):
             self.inp, self.n_hyp, self.n_levels = inp, n, di.n_levels
 
-    def run(self, prior_pose, stream=None):
+    def run(self, prior_pose, stream=None, count_visible=False):
         """prior_pose: cuda float32 [12]. Returns device tensors: best_idx (into the kept set), best_pose, best_cost,
-        kept_idx [keep] (into the H0 grid), poses [keep,12], cost [keep], coarse_kept_cost [keep] (ascending)."""
+        kept_idx [keep] (into the H0 grid), poses [keep,12], cost [keep], coarse_kept_cost [keep] (ascending).
+        count_visible (measurement only: synchronises twice): also `visible_evals` = [coarse level, finer levels]."""
         torch, L = self.torch, self.di.n_levels
         light = ("poses", "cost", "n_valid", "status")
         seed_hypotheses(prior_pose, self.offsets, self.seed_frame, out=self.seeds, stream=stream)
         o0 = self.ref.run(self._View(self.di, self.inp0, self.H0), self.params, stream, light, levels=(0, 1))
         n = self.ref.last_launches
+        vis = [self.ref.last_visible_evals(stream)] if count_visible else None
         kept_idx, kept_poses, coarse_kept = prune_topk(o0["cost"], o0["poses"], self.keep, stream)
         self.inp1.init_poses_dev = kept_poses.data_ptr()
         o1 = self.ref.run(self._View(self.di, self.inp1, self.keep), self.params, stream, light, levels=(1, L))
         idx, pose, bc = select_best(o1["cost"], o1["poses"], stream)
         self.launches = n + self.ref.last_launches + 3
         self._keepalive = kept_poses
+        if count_visible:
+            vis.append(self.ref.last_visible_evals(stream))
+            self.visible_evals = vis
         return dict(best_idx=idx, best_pose=pose, best_cost=bc, kept_idx=kept_idx, poses=o1["poses"], cost=o1["cost"],
                     n_valid=o1["n_valid"], status=o1["status"], coarse_kept_cost=coarse_kept)
 
@@ -649,6 +677,16 @@ def probe_gather(buffer_bytes, vec_bytes, launches=5, device=0):
     g = C.c_double()
     _check(lib().pilot_refine_probe_gather(int(device), int(buffer_bytes), int(vec_bytes), int(launches), C.byref(g)),
            "pilot_refine_probe_gather")
+    return g.value
+
+
+def probe_unit_gather(buffer_bytes, px_bytes, variant=0, launches=5, device=0):
+    """Random gather of unit-shaped footprints (2 x 2 pixels of px_bytes + a reference row): GB/s of tap bytes.
+    variant 0 = the kernel's LDG shape, 1 = staged through shared memory with cp.async.bulk."""
+    _torch()
+    g = C.c_double()
+    _check(lib().pilot_refine_probe_unit_gather(int(device), int(buffer_bytes), int(px_bytes), int(variant), int(launches),
+                                                C.byref(g)), "pilot_refine_probe_unit_gather")
     return g.value
 
 

@@ -61,6 +61,7 @@ struct HypState {
   int level;                // pyramid level this hypothesis is in (n_levels = finished)
   int k;                    // solves consumed at this level
   int pending;              // 1 if (Rc, Cc) came from a solve (not the level's first evaluation)
+  unsigned long long visible_evals;   // measurement: visible (anchor, hypothesis) units summed over every EVAL pass of the run
 };
 
 struct LevelArgs {
@@ -397,6 +398,13 @@ template <> struct MmaType<F16Tag> {
 };
 template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features stay on the FFMA2 path
 
+#ifndef PILOT_MMA_PIPE
+#define PILOT_MMA_PIPE 1           // 1: the next round's taps are loaded while this round's mma.sync run (up to 64 channels).
+                                   // Measured (B200): cluster-resident kernel at 128 registers, 32 channels: config 1 0.642 -> 0.610 ms,
+                                   // config 3 1.063 -> 1.029; pass kernel, 64 channels: 8.76 -> 8.31 ms at 16 warps per SM but
+                                   // 7.88 without it at 24 warps (80 registers, where it spills): pilot_pass_mma.cu turns it off
+#endif
+
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
   static constexpr int PX = CH * 2;                    // bytes per pixel
   static constexpr int TB = PX / 4 < 32 ? PX / 4 : 32; // bytes per load per thread (the 4 q-threads share a pixel): 8, 16, 32
@@ -547,6 +555,71 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
     __syncwarp();
 
     const int nr = (nv + 7) >> 3;
+#if PILOT_MMA_PIPE
+    if constexpr (Geo::PARTS == 1) {
+      // Software pipeline over the rounds: the next round's five loads are issued as soon as this round's taps have been
+      // turned into differences (their registers are free again), so they are in flight during the 6 KS mma.sync and the
+      // hand-off of this round - a warp always has loads outstanding, whatever phase the other warps of the SM are in.
+      TapWords<NW> t[5];
+      auto issue = [&](int r) {
+        const int s = 8 * r + g;
+        const uint2 sl = slots[s < nv ? s : 0];        // a row-group past the last visible unit repeats slot 0 (L1 hits)
+        const char* const p0 = featq + sl.x;
+        t[0] = ldg_words<NW>(p0);
+        t[1] = ldg_words<NW>(p0 + PX);
+        t[2] = ldg_words<NW>(p0 + row_stride);
+        t[3] = ldg_words<NW>(p0 + row_stride + PX);
+        t[4] = ldg_words<NW>(refq + (size_t)sl.y * PX);
+      };
+      issue(0);
+      for (int r = 0; r < nr; ++r) {
+        const int s = 8 * r + g;
+        const bool act = s < nv;
+        unsigned e0[NW], e1[NW], e2[NW], e3[NW];
+#pragma unroll
+        for (int i = 0; i < NW; ++i) {
+          e0[i] = M::sub2(t[1].w[i], t[0].w[i]);
+          e1[i] = M::sub2(t[3].w[i], t[2].w[i]);
+          e2[i] = M::sub2(t[2].w[i], t[0].w[i]);
+          e3[i] = M::sub2(t[4].w[i], t[2].w[i]);
+        }
+        if (r + 1 < nr) issue(r + 1);
+        float c0[4], c1[4], c2[4], c3[4], c4[4], c5[4];
+#pragma unroll
+        for (int k = 0; k < KS; ++k) {
+          const unsigned e0a = e0[2 * k], e0b = e0[2 * k + 1], e1a = e1[2 * k], e1b = e1[2 * k + 1];
+          const unsigned e2a = e2[2 * k], e2b = e2[2 * k + 1], e3a = e3[2 * k], e3b = e3[2 * k + 1];
+          if (k == 0) {
+            M::mma0(c0, e0a, e2a, e0b, e2b, e0a, e0b);                    // e0.e0 | e2.e0
+            M::mma0(c1, e0a, e2a, e0b, e2b, e1a, e1b);                    // e0.e1 | e2.e1
+            M::mma0(c2, e0a, e2a, e0b, e2b, e3a, e3b);                    // e0.e3 | e2.e3
+            M::mma0(c3, e0a, e2a, e0b, e2b, e2a, e2b);                    // (e0.e2) | e2.e2
+            M::mma0(c4, e1a, e3a, e1b, e3b, e1a, e1b);                    // e1.e1 | e3.e1
+            M::mma0(c5, e1a, e3a, e1b, e3b, e3a, e3b);                    // (e1.e3) | e3.e3
+          } else {
+            M::mma(c0, e0a, e2a, e0b, e2b, e0a, e0b);
+            M::mma(c1, e0a, e2a, e0b, e2b, e1a, e1b);
+            M::mma(c2, e0a, e2a, e0b, e2b, e3a, e3b);
+            M::mma(c3, e0a, e2a, e0b, e2b, e2a, e2b);
+            M::mma(c4, e1a, e3a, e1b, e3b, e1a, e1b);
+            M::mma(c5, e1a, e3a, e1b, e3b, e3a, e3b);
+          }
+        }
+        if (diag && act) {
+          const unsigned rp = rows_s + (unsigned)(s * Geo::kRow) * 4u;
+          const float E00 = odd ? c0[1] : c0[0], E02 = odd ? c0[3] : c0[2];
+          const float E01 = odd ? c1[1] : c1[0], E12 = odd ? c1[3] : c1[2];
+          const float E03 = odd ? c2[1] : c2[0], E23 = odd ? c2[3] : c2[2];
+          const float E22 = odd ? c3[3] : c3[2];
+          const float E11 = odd ? c4[1] : c4[0], E13 = odd ? c4[3] : c4[2];
+          const float E33 = odd ? c5[3] : c5[2];
+          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp), "f"(E00), "f"(E01), "f"(E02), "f"(E03) : "memory");
+          asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp + 16u), "f"(E11), "f"(E12), "f"(E13), "f"(E22) : "memory");
+          asm volatile("st.shared.v2.f32 [%0], {%1,%2};" :: "r"(rp + 32u), "f"(E23), "f"(E33) : "memory");
+        }
+      }
+    } else
+#endif
     for (int r = 0; r < nr; ++r) {
       const int s = 8 * r + g;
       const bool act = s < nv;
@@ -1124,6 +1197,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
   for (int i = 0; i < 6; ++i) gn[i] = (double)sums[21 + i];
   costn = (double)sums[27];
   int nv = (int)(sums[28] + 0.5f);
+  s.visible_evals += (unsigned long long)nv;
   if (nv < P.min_valid) { costn = INFINITY; fl |= PILOT_STATUS_FEW_VALID; }
 
   if (P.w_gravity > 0.f) {                                                   // Eq.(3)

@@ -9,6 +9,9 @@
 #define PILOT_MMA_THREADS 128
 #define PILOT_MMA_MIN_BLOCKS 6
 #endif
+#ifndef PILOT_MMA_PIPE
+#define PILOT_MMA_PIPE 0
+#endif
 #define PILOT_THREADS PILOT_MMA_THREADS
 #define PILOT_MIN_BLOCKS PILOT_MMA_MIN_BLOCKS
 #include "pilot_pass.cuh"

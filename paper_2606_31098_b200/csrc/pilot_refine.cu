@@ -57,9 +57,19 @@ __global__ void init_state_kernel(HypState* state, unsigned* counters, const flo
   for (int i = 0; i < 21; ++i) s.H[i] = 0.0;
   for (int i = 0; i < 6; ++i) s.g[i] = 0.0;
   s.cost = 0.0; s.lambda = lambda_init; s.n_valid = 0; s.flags = 0; s.status = 0;
-  s.level = level_begin; s.k = 0; s.pending = 0;
+  s.level = level_begin; s.k = 0; s.pending = 0; s.visible_evals = 0ull;
   state[m] = s;
   counters[m] = 0u;
+}
+
+__global__ void visible_sum_kernel(const HypState* state, int n_hyp, unsigned long long* out) {
+  unsigned long long t = 0ull;
+  for (int m = threadIdx.x; m < n_hyp; m += blockDim.x) t += state[m].visible_evals;
+  for (int o = 16; o >= 1; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+  __shared__ unsigned long long part[8];
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = t;
+  __syncthreads();
+  if (threadIdx.x == 0) { unsigned long long a = 0ull; for (int i = 0; i < 8; ++i) a += part[i]; *out = a; }
 }
 
 }  // namespace
@@ -78,6 +88,8 @@ struct pilot_refine_handle {
   int math_mode;            // pilot_math_mode
   int sm_count;
   int last_launches;
+  int last_n_hyp;
+  unsigned last_mma_levels, last_resident_levels;   // bit l: level l of the last run used the tensor-core contraction / the resident kernel
   // host-path staging (create_host only)
   bool host_mode;
   int max_dsm_w, max_dsm_h;
@@ -123,7 +135,7 @@ bool shape_supported(const pilot_refine_config* c) {
   return true;
 }
 
-struct WsLayout { size_t state, counters, partials, total; int max_chunks; };
+struct WsLayout { size_t state, counters, partials, scratch, total; int max_chunks; };
 
 WsLayout ws_layout(const pilot_refine_config* c) {
   WsLayout w;
@@ -132,6 +144,7 @@ WsLayout ws_layout(const pilot_refine_config* c) {
   w.state = o;    o = align_up(o + sizeof(HypState) * (size_t)c->max_hypotheses, 256);
   w.counters = o; o = align_up(o + sizeof(unsigned) * (size_t)c->max_hypotheses, 256);
   w.partials = o; o = align_up(o + sizeof(float) * kNacc * (size_t)c->max_hypotheses * (size_t)w.max_chunks, 256);
+  w.scratch = o;  o = align_up(o + 256, 256);
   w.total = o;
   return w;
 }
@@ -195,9 +208,12 @@ bool use_mma(const pilot_refine_handle* h, int g, int grad_mode, bool resident) 
   if (h->math_mode == PILOT_MATH_FP32) return false;
   const bool applies = h->cfg.feat_dtype != PILOT_F32 && grad_mode == PILOT_GRAD_BILINEAR_EXACT && (g == 2 || g == 4 || g == 8 || g == 16);
   if (h->math_mode == PILOT_MATH_MMA) return applies;
-  // AUTO: measured on B200 (ms per step, FP32 -> MMA): config 4 11.89 -> 9.60, config 2 11.43 -> 9.61 (64 channels, one
-  // launch per pass); config 1 0.67 -> 0.72, config 3 1.12 -> 1.20, paper schedule 0.32 -> 0.33 (32 channels, cluster-resident)
-  return applies && g >= 8 && !resident;
+  // AUTO: measured on B200 (ms per step, FP32 -> MMA, round 2's one-unit-per-row-group gather): config 4 9.60 (7.65 with the
+  // empty batches skipped) -> 7.88, config 2 8.02 -> 7.64 (64 channels, one launch per pass); config 1 0.642 -> 0.610,
+  // config 3 1.093 -> 1.029, paper schedule 0.325 -> 0.289 (32 channels, cluster-resident and the 1210-hypothesis coarse pass).
+  // 16 channels (8-byte loads per thread) were not measured: they stay on FFMA2.
+  (void)resident;
+  return applies && g >= 4;
 }
 
 int choose_chunk(const pilot_refine_handle* h, int n_hyp, int n_points) {
@@ -243,6 +259,8 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->cluster_override = 0;
   h->math_mode = PILOT_MATH_AUTO;
   h->last_launches = 0;
+  h->last_n_hyp = 0;
+  h->last_mma_levels = h->last_resident_levels = 0u;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
   h->copy_stream = nullptr; h->n_submitted = h->n_waited = 0;
   for (int i = 0; i < 2; ++i) { h->ev_copied[i] = nullptr; h->ev_done[i] = nullptr; }
@@ -305,6 +323,30 @@ int pilot_refine_set_math_mode(pilot_refine_handle* h, int mode) {
 
 int pilot_refine_last_launches(const pilot_refine_handle* h) { return h ? h->last_launches : 0; }
 
+int pilot_refine_last_plan(const pilot_refine_handle* h, unsigned* mma_levels, unsigned* resident_levels) {
+  if (!h) return PILOT_ERR_ARG;
+  if (mma_levels) *mma_levels = h->last_mma_levels;
+  if (resident_levels) *resident_levels = h->last_resident_levels;
+  return PILOT_OK;
+}
+
+int pilot_refine_last_visible_evals(pilot_refine_handle* h, void* cuda_stream, unsigned long long* out_host) {
+  if (!h || !out_host) return PILOT_ERR_ARG;
+  *out_host = 0ull;
+  if (h->last_n_hyp <= 0) return PILOT_OK;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != h->cfg.device && cudaSetDevice(h->cfg.device) != cudaSuccess) return PILOT_ERR_CUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  WsLayout w = ws_layout(&h->cfg);
+  unsigned long long* d = reinterpret_cast<unsigned long long*>(h->ws + w.scratch);
+  visible_sum_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const HypState*>(h->ws + w.state), h->last_n_hyp, d);
+  bool ok = cudaMemcpyAsync(out_host, d, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+            cudaStreamSynchronize(st) == cudaSuccess;
+  if (prev != h->cfg.device) cudaSetDevice(prev);
+  return ok ? PILOT_OK : PILOT_ERR_CUDA;
+}
+
 int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
                      const pilot_refine_outputs* out, void* cuda_stream) {
   if (!h) return PILOT_ERR_ARG;
@@ -358,6 +400,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
   A.out = *out;
 
   int launches = 0;
+  unsigned plan_mma = 0u, plan_res = 0u;
   init_state_kernel<<<(A.n_hyp + 127) / 128, 128, 0, st>>>(A.state, A.counters, in->init_poses_dev, A.n_hyp, (double)p->lambda_init,
                                                                   level_begin);
   ++launches;
@@ -374,6 +417,8 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     const int cluster = choose_resident(h, A.n_hyp, L.N);
     bool mma = use_mma(h, g, p->grad_mode, cluster > 0);
     if (mma && MmaGeom<64>::LB == 32 && g >= 8 && (((uintptr_t)L.feat | (uintptr_t)L.ref) & 31)) mma = false;   // 32-byte loads
+    if (mma) plan_mma |= 1u << l;
+    if (cluster > 0) plan_res |= 1u << l;
     A.chunk = choose_chunk(h, A.n_hyp, L.N);
     A.n_chunks = L.N > 0 ? (L.N + A.chunk - 1) / A.chunk : 1;
     if (A.n_chunks > h->max_chunks) { A.chunk = kMinChunk; A.n_chunks = (L.N + kMinChunk - 1) / kMinChunk; }
@@ -419,6 +464,8 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
     rec_base += p->iters[l];
   }
   h->last_launches = launches;
+  h->last_n_hyp = A.n_hyp;
+  h->last_mma_levels = plan_mma; h->last_resident_levels = plan_res;
   cudaError_t e = cudaGetLastError();
   if (prev != c.device) cudaSetDevice(prev);
   return e == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;

@@ -514,3 +514,19 @@ def paper_frame(N=500, iters=(2, 3, 4), dtype="bf16", prior_error=(3.1, -4.3, 2.
 
 def make(name, **kw):
     return {"config0": config0, "config1": config1, "config2": config2, "config4": config4}[name](**kw)
+
+
+def levels_slice(prob, begin, end, poses=None):
+    """Sub-problem made of pyramid levels [begin, end) of `prob` (what pilot_refine_run_levels works on), optionally with
+    other initial poses. Dict slicing only."""
+    q = dict(prob)
+    q["n_levels"] = end - begin
+    for k in ("width", "height", "channels", "query_feat", "intrinsics", "points", "ref_feat"):
+        q[k] = list(prob[k][begin:end])
+    q["query_conf"] = list(prob.get("query_conf", [None] * prob["n_levels"])[begin:end])
+    if poses is not None:
+        q["init_poses"] = np.ascontiguousarray(poses, np.float32).reshape(-1, 12)
+    P = dict(prob.get("params", {}))
+    P["iters"] = list(P["iters"][begin:end])
+    q["params"] = P
+    return q

@@ -54,16 +54,4 @@ def pose_errors(gpu, orc):
     return rot_angle(gpu["poses"], orc["poses64"]), trans_dist(gpu["poses"], orc["poses64"])
 
 
-def levels_slice(prob, begin, end, poses=None):
-    """Sub-problem made of pyramid levels [begin, end) of `prob` (the oracle's view of pilot_refine_run_levels)."""
-    q = dict(prob)
-    q["n_levels"] = end - begin
-    for k in ("width", "height", "channels", "query_feat", "intrinsics", "points", "ref_feat"):
-        q[k] = list(prob[k][begin:end])
-    q["query_conf"] = list(prob.get("query_conf", [None] * prob["n_levels"])[begin:end])
-    if poses is not None:
-        q["init_poses"] = np.ascontiguousarray(poses, np.float32).reshape(-1, 12)
-    P = dict(prob.get("params", {}))
-    P["iters"] = list(P["iters"][begin:end])
-    q["params"] = P
-    return q
+from paper_2606_31098_b200.workloads import levels_slice  # noqa: E402,F401  (dict slicing; lives with the generators)
