@@ -405,6 +405,10 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
                                    // 7.88 without it at 24 warps (80 registers, where it spills): pilot_pass_mma.cu turns it off
 #endif
 
+#ifndef PILOT_MMA_SB
+#define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
+                                    // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
+#endif
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
   static constexpr int PX = CH * 2;                    // bytes per pixel
   static constexpr int TB = PX / 4 < 32 ? PX / 4 : 32; // bytes per load per thread (the 4 q-threads share a pixel): 8, 16, 32
@@ -415,8 +419,11 @@ template <int CH> struct MmaGeom {            // CH = channels of a 16-bit featu
   static constexpr int kRow = 12;                      // floats per unit row of the warp's hand-off buffer: the ten distinct
                                                        // entries of E + 2 pad; 8 consecutive rows x 16 B fall in 8 distinct
                                                        // groups of four banks (12 i mod 32 = 0,12,24,4,16,28,8,20)
-  static constexpr int kSlotFloats = 64;               // 32 x {tap offset, anchor index in the batch}
-  static constexpr int kWarpFloats = kSlotFloats + 32 * kRow;
+  static constexpr int SB = PILOT_MMA_SB;              // anchors per super-batch of a warp (a multiple of 32)
+  // the warp's buffer, per slot of the super-batch: {tap offset, anchor index} (8 B, read by the rounds), {a, b, X/Z, Y/Z}
+  // (16 B) and {1/Z, w_ref} (8 B) (read by the lane phase), and the Gram row (kRow floats)
+  static constexpr int kSlotA = 0, kSlotB = 2 * SB, kSlotC = 6 * SB, kRows = 8 * SB;
+  static constexpr int kWarpFloats = 8 * SB + SB * kRow;
 };
 template <int G> __host__ __device__ constexpr bool mma_supported() { return G == 2 || G == 4 || G == 8 || G == 16; }
 
@@ -476,14 +483,15 @@ template <int G, bool MMA> constexpr size_t gather_smem_bytes() {
 
 // ------------------------------------------------------------------ the photo gather, tensor-core contraction
 //
-// Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on batches of 32 anchors:
-//   lane-per-unit   anchor load (one batch ahead), projection + visibility in fp64 (a2); the VISIBLE units of the batch are
-//                   compacted (ballot + popc rank): their tap offset and anchor index go to slot `rank` of the warp's table,
-//                   a batch with no visible unit is skipped, and only ceil(n_visible / 8) rounds run;
-//   fragment roles  per round, row-group g takes slot 8 r + g: five loads, four packed differences per word,
-//                   6 KS mma.sync; thread (g, g / 2) hands the unit's ten Gram entries to row `slot` of the warp's buffer;
-//   lane-per-unit   the unit's own lane reads its row: Gram -> six scalars, robust weight, lift through J_uv, and the batch is
-//                   reduce-scattered over the warp into one accumulator register per lane (a4-a6).
+// Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on super-batches of SB
+// anchors (SB / 32 of its round-robin batches), in three phases:
+//   project    lane-per-anchor, SB / 32 passes: anchor load, projection + visibility in fp64 (a2). The VISIBLE units are
+//              compacted (ballot + popc rank, running count): slot s of the warp's table gets {tap offset, anchor index} and
+//              the lane-phase state {a, b, X/Z, Y/Z, 1/Z, w_ref}; invisible anchors cost nothing beyond this point;
+//   rounds     ceil(n_visible / 8) rounds; row-group g takes slot 8 r + g: five loads, four packed differences per word,
+//              6 KS mma.sync; thread (g, g / 2) hands the unit's ten Gram entries to row `slot` of the warp's buffer;
+//   lift       lane i takes slots i, i + 32, ...: Gram -> six scalars, robust weight, lift through J_uv into 29 registers
+//              (a4-a5); ONE reduce-scatter per super-batch leaves component i of the warp's total in lane i (a6).
 template <class T, int G>
 __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const double* Rc, const double* Ccand,
                                                      int begin, int end, int worker, int n_workers,
@@ -491,7 +499,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   constexpr int CH = 8 * G;
   using Geo = MmaGeom<CH>;
   using M = MmaType<T>;
-  constexpr int NW = Geo::NW, PX = Geo::PX, KS = Geo::KS;
+  constexpr int NW = Geo::NW, PX = Geo::PX, KS = Geo::KS, SB = Geo::SB;
   const LevelArgs& L = A.lv;
   const int lane = threadIdx.x & 31;
   const unsigned row_stride = (unsigned)PX * (unsigned)L.W;
@@ -508,52 +516,61 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const bool odd = g & 1;                                                 // ... in c[1], c[3] (else c[0], c[2])
   const char* const featq = feat + q * Geo::TB;
   const char* const refq = refb + q * Geo::TB;
-  uint2* const slots = reinterpret_cast<uint2*>(red);
-  float* const rows = red + Geo::kSlotFloats;
+  uint2* const slotA = reinterpret_cast<uint2*>(red + Geo::kSlotA);
+  float4* const slotB = reinterpret_cast<float4*>(red + Geo::kSlotB);
+  float2* const slotC = reinterpret_cast<float2*>(red + Geo::kSlotC);
+  float* const rows = red + Geo::kRows;
   const unsigned rows_s = (unsigned)__cvta_generic_to_shared(rows);
 
-  struct Unit { float a, b, X, Y, iz, w; unsigned off; bool valid; };
-  auto load_anchor = [&](int base) { const int j = base + lane; return j < end ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
-  auto project = [&](const float4& P, int base) {                         // a2, in double so that u, v carry no fp32 noise
-    Unit U;
-    bool valid = base + lane < end;
-    double R[12];                                                         // six 16-byte shared-memory loads
-#pragma unroll
-    for (int i = 0; i < 6; ++i)
-      asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
-    const double* Cc = R + 9;
-    double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
-    double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
-    double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
-    double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
-    valid = valid && (Zd > (double)A.prm.z_near);
-    double izd = fast_rcp(Zd);
-    double ud = (double)L.fx * Xd * izd + (double)L.cx;
-    double vd = (double)L.fy * Yd * izd + (double)L.cy;
-    double x0d = floor(ud), y0d = floor(vd);
-    valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
-    U.a = valid ? (float)(ud - x0d) : 0.f;
-    U.b = valid ? (float)(vd - y0d) : 0.f;
-    const int x0 = valid ? (int)x0d : 0, y0 = valid ? (int)y0d : 0;
-    U.off = ((unsigned)y0 * (unsigned)L.W + (unsigned)x0) * (unsigned)PX;
-    U.X = (float)Xd; U.Y = (float)Yd; U.iz = (float)izd; U.w = P.w; U.valid = valid;
-    return U;
-  };
 
-  const int step = n_workers * 32;
-  int base = begin + worker * 32;
-  if (base >= end) return;
-  float4 Pn = load_anchor(base);
-  for (; base < end; base += step) {
-    const Unit cur = project(Pn, base);
-    Pn = load_anchor(base + step);                                        // next batch's anchors: in flight during this batch
-    const unsigned vmask = __ballot_sync(0xffffffffu, cur.valid);
-    if (vmask == 0u) continue;                                            // no visible unit in this batch: nothing to gather
-    const int nv = __popc(vmask);
-    const int rank = __popc(vmask & ((1u << lane) - 1u));
-    if (cur.valid) slots[rank] = make_uint2(cur.off, (unsigned)(base + lane));
+  // The 32-anchor batches of [begin, end) go round-robin over the workers (batch b to worker b mod n_workers: the warps that
+  // run together sweep neighbouring anchors, which is what keeps the union of the resident CTAs' footprints in L2); a
+  // worker takes its batches SB / 32 at a time.
+  const int n_batches = (end - begin + 31) >> 5;
+  auto load_anchor = [&](int b) { const int j = begin + b * 32 + lane; return (b < n_batches && j < end) ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
+  constexpr int PASSES = SB / 32;
+  for (int b0 = worker; b0 < n_batches; b0 += PASSES * n_workers) {
+    // ---- project + compact
+    int nv = 0;
+    float4 Pn = load_anchor(b0);
+#pragma unroll 1
+    for (int k = 0; k < PASSES; ++k) {
+      const int b = b0 + k * n_workers;
+      if (b >= n_batches) break;
+      const int base = begin + b * 32;
+      const float4 P = Pn;
+      Pn = load_anchor(b + n_workers);                                    // next pass's anchors: in flight during this one
+      bool valid = base + lane < end;
+      double R[12];                                                       // six 16-byte shared-memory loads
+#pragma unroll
+      for (int i = 0; i < 6; ++i)
+        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
+      const double* Cc = R + 9;
+      double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
+      double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
+      double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
+      double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
+      valid = valid && (Zd > (double)A.prm.z_near);
+      double izd = fast_rcp(Zd);
+      double ud = (double)L.fx * Xd * izd + (double)L.cx;
+      double vd = (double)L.fy * Yd * izd + (double)L.cy;
+      double x0d = floor(ud), y0d = floor(vd);
+      valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
+      const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+      if (valid) {
+        const int s = nv + __popc(vmask & ((1u << lane) - 1u));
+        const unsigned off = ((unsigned)(int)y0d * (unsigned)L.W + (unsigned)(int)x0d) * (unsigned)PX;
+        const float iz = (float)izd;
+        slotA[s] = make_uint2(off, (unsigned)(base + lane));
+        slotB[s] = make_float4((float)(ud - x0d), (float)(vd - y0d), (float)Xd * iz, (float)Yd * iz);
+        slotC[s] = make_float2(iz, P.w);
+      }
+      nv += __popc(vmask);
+    }
+    if (nv == 0) continue;                                                // no visible unit: nothing to gather
     __syncwarp();
 
+    // ---- rounds
     const int nr = (nv + 7) >> 3;
 #if PILOT_MMA_PIPE
     if constexpr (Geo::PARTS == 1) {
@@ -563,7 +580,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       TapWords<NW> t[5];
       auto issue = [&](int r) {
         const int s = 8 * r + g;
-        const uint2 sl = slots[s < nv ? s : 0];        // a row-group past the last visible unit repeats slot 0 (L1 hits)
+        const uint2 sl = slotA[s < nv ? s : 0];        // a row-group past the last visible unit repeats slot 0 (L1 hits)
         const char* const p0 = featq + sl.x;
         t[0] = ldg_words<NW>(p0);
         t[1] = ldg_words<NW>(p0 + PX);
@@ -625,7 +642,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       const bool act = s < nv;
       float c0[4], c1[4], c2[4], c3[4], c4[4], c5[4];
       // a row-group past the last visible unit repeats slot 0 (always there: its loads hit L1) and stores nothing
-      const uint2 sl = slots[act ? s : 0];
+      const uint2 sl = slotA[act ? s : 0];
       const char* const p0 = featq + sl.x;
       const char* const pr = refq + (size_t)sl.y * PX;
 #pragma unroll
@@ -673,26 +690,27 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
     }
     __syncwarp();
 
-    // ---- lane-per-unit: Gram -> six scalars, robust weight, lift through the 2x6 Jacobian (a4-a6)
+    // ---- lift: lane-per-unit over the compacted slots (a4-a5), one reduce-scatter per super-batch (a6)
     float v[32];
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = 0.f;
-    if (cur.valid) {
-      const float a = cur.a, b = cur.b;
+    for (int s = lane; s < nv; s += 32) {
+      const float4 sb4 = slotB[s];
+      const float2 sc2 = slotC[s];
+      const float a = sb4.x, b = sb4.y, x = sb4.z, y = sb4.w, iz = sc2.x;
       float p[6];
-      gram_unit_scalars(rows + rank * Geo::kRow, a, b, p);
+      gram_unit_scalars(rows + s * Geo::kRow, a, b, p);
       float wq = 1.f;
       if (L.conf) {
-        const float* cq = L.conf + cur.off / (unsigned)PX;
+        const float* cq = L.conf + slotA[s].x / (unsigned)PX;
         float q00 = __ldg(cq), q10 = __ldg(cq + 1), q01 = __ldg(cq + L.W), q11 = __ldg(cq + L.W + 1);
         wq = (1.f - b) * ((1.f - a) * q00 + a * q10) + b * ((1.f - a) * q01 + a * q11);
       }
-      float w = cur.w * wq;
+      float w = sc2.y * wq;
       float rho, drho;
       robust_fast(A.prm.loss, w * p[5], A.prm.loss_scale, rho, drho);
       float om = w * drho;
-      float x = cur.X * cur.iz, y = cur.Y * cur.iz;
-      float fxz = L.fx * cur.iz, fyz = L.fy * cur.iz;
+      float fxz = L.fx * iz, fyz = L.fy * iz;
       float Ju[6] = {fxz, 0.f, -fxz * x, -L.fx * x * y, L.fx * (1.f + x * x), -L.fx * y};
       float Jv[6] = {0.f, fyz, -fyz * y, -L.fy * (1.f + y * y), L.fy * x * y, L.fy * x};
       float A11 = om * p[0], A12 = om * p[1], A22 = om * p[2];
@@ -702,15 +720,15 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
         float mu = A11 * Ju[i] + A12 * Jv[i];
         float mv = A12 * Ju[i] + A22 * Jv[i];
 #pragma unroll
-        for (int k = i; k < 6; ++k) v[tri(i, k)] = mu * Ju[k] + mv * Jv[k];
-        v[21 + i] = b1 * Ju[i] + b2 * Jv[i];
+        for (int k = i; k < 6; ++k) v[tri(i, k)] += mu * Ju[k] + mv * Jv[k];
+        v[21 + i] += b1 * Ju[i] + b2 * Jv[i];
       }
-      v[27] = rho;
-      v[28] = 1.f;
+      v[27] += rho;
+      v[28] += 1.f;
     }
-    __syncwarp();                                                         // rows and slots are rewritten by the next batch
-    // reduce-scatter of the batch over the warp: lane i ends with the batch total of component i (31 shuffles), which
-    // goes to ONE accumulator register per lane: no shared-memory traffic, no 29 live registers
+    __syncwarp();                                                         // the table is rewritten by the next super-batch
+    // reduce-scatter over the warp: lane i ends with the super-batch total of component i (31 shuffles), which goes to ONE
+    // accumulator register per lane
 #pragma unroll
     for (int half = 16; half >= 1; half >>= 1) {
       const bool upper = lane & half;

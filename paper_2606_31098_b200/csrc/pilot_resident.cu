@@ -13,6 +13,9 @@
 // whole level; launches, grid ramps, the atomic ticket and the global partial sums of the pass kernel disappear.
 //
 // Shares no code with oracle/.
+#ifndef PILOT_MMA_SB
+#define PILOT_MMA_SB 128            // anchors per super-batch of a warp (10 KB of shared memory per warp at 2 CTAs per SM)
+#endif
 #include "pilot_device.cuh"
 
 #include <cooperative_groups.h>
@@ -51,10 +54,11 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
   const ResidentShared* master = cluster.map_shared_rank(&sh, 0);
   const bool range_on = range_enabled(A);
   const bool prior_warp = range_on && rank == 0 && warp == kWarps - 1;
-  const int n_workers = (range_on && rank == 0) ? kWarps - 1 : kWarps;
+  // the gathering warps of the whole cluster share the anchors: worker w of n_workers (rank 0's last warp evaluates the
+  // range prior instead) - contiguous equal ranges on the tensor-core path, 32-anchor batches round-robin on the FFMA2 path
+  const int n_workers = (int)S * kWarps - (range_on ? 1 : 0);
+  const int worker = (int)rank * kWarps + warp - ((range_on && rank > 0) ? 1 : 0);
   const int N = A.lv.N;
-  const int per = (((N + (int)S - 1) / (int)S) + 31) / 32 * 32;      // anchors per CTA, whole 32-unit batches
-  const int begin = min((int)rank * per, N), end = min(begin + per, N);
 
 #ifdef PILOT_RESIDENT_PROFILE
   long long t_eval = 0, t_fin = 0, t_red = 0, t_all = clock64(), t0 = 0, n_it = 0;
@@ -78,7 +82,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
         for (int i = 0; i < 6; ++i) sh.prior.J[i] = ok ? Jr[i] : 0.0;
       }
     } else {
-      photo_accumulate<T, G, CEN, MMA>(A, sh.pose, sh.pose + 9, begin, end, warp, n_workers, acc, sacc, red);
+      photo_accumulate<T, G, CEN, MMA>(A, sh.pose, sh.pose + 9, 0, N, worker, n_workers, acc, sacc, red);
     }
     const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
 #ifdef PILOT_RESIDENT_PROFILE
