@@ -111,6 +111,8 @@ class Resident:
         self.prob = prob = make_problem(args.config, rank)
         self.params = prob["params"]
         self.di = binding.DeviceInputs(prob, local_rank)
+        if getattr(args, "sort_anchors", False):
+            self.di.sort_anchors()                       # pilot_refine_sort_anchors: Morton order on the device
         self.ref = binding.Refiner.for_inputs(self.di, self.params, local_rank)
         if args.chunk:
             self.ref.set_chunk(args.chunk)
@@ -622,6 +624,8 @@ def main():
     ap.add_argument("--cluster", type=int, default=0, help="CTAs per hypothesis of the resident kernel (0 = heuristic)")
     ap.add_argument("--shuffle-anchors", action="store_true", help="hand the anchors over in a random order instead of the "
                     "generator's Morton order (config1/2/4): measures what the caller's ordering is worth")
+    ap.add_argument("--sort-anchors", action="store_true", help="put the anchors in Morton order with pilot_refine_sort_anchors "
+                    "before the timed region (with --shuffle-anchors: what the library's own ordering recovers)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the gather-peak micro-benchmark")
@@ -646,7 +650,7 @@ def main():
     stream = torch.cuda.current_stream(local_rank)
     l2_bytes = torch.cuda.get_device_properties(local_rank).L2_cache_size
     hbm = load_peaks()
-    default_run = args.config == "config4" and world == 1 and not args.no_others and not args.shuffle_anchors
+    default_run = args.config == "config4" and world == 1 and not args.no_others and not args.shuffle_anchors and not args.sort_anchors
     peaks = None
     if rank == 0 and not args.no_probe:
         peaks = gather_peaks(binding, [64, 128] if default_run else [128 if args.config in ("config2", "config4") else 64], local_rank)
@@ -670,8 +674,9 @@ def main():
         cfg = main_res["config"]
         cfg["sharding"] = ("hypotheses across ranks, no data-path collective; one 13-float-per-hypothesis "
                            "all-gather + arg-min ends the step when n_gpus > 1")
-        if args.shuffle_anchors:
-            cfg["anchor_order"] = "random permutation (--shuffle-anchors)"
+        if args.shuffle_anchors or args.sort_anchors:
+            cfg["anchor_order"] = ("random permutation (--shuffle-anchors)" if args.shuffle_anchors else "generator's order") + \
+                (", then pilot_refine_sort_anchors (Morton order on the device)" if args.sort_anchors else "")
         line = {"metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": main_res["warmup"], "ms_per_step": main_res["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": main_res["dtype"], "data": "synthetic", "config": cfg,

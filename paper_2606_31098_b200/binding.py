@@ -34,6 +34,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
            "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
            "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
+           "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
            "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
@@ -172,6 +173,11 @@ def lib():
         L.pilot_refine_last_visible_evals.restype = C.c_int
         L.pilot_refine_last_plan.argtypes = [C.c_void_p, C.POINTER(C.c_uint), C.POINTER(C.c_uint)]
         L.pilot_refine_last_plan.restype = C.c_int
+        L.pilot_refine_sort_anchors_temp_bytes.argtypes = [C.c_int]
+        L.pilot_refine_sort_anchors_temp_bytes.restype = C.c_size_t
+        L.pilot_refine_sort_anchors.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                                C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+        L.pilot_refine_sort_anchors.restype = C.c_int
         for name in EXPORTS:
             if name.startswith("pilot_refine_sequence_"):
                 getattr(L, name).restype = C.c_int
@@ -267,6 +273,34 @@ class DeviceInputs:
         inp.dsm_gsd = float(prob["dsm_gsd"])
         self.inp = inp
         self.max_points = max(int(inp.n_points[l]) for l in range(L))
+
+    def sort_anchors(self, stream=None):
+        """Put every level's anchors and reference rows in Morton order on the device (pilot_refine_sort_anchors) and
+        point the Inputs struct at the sorted copies. Returns the permutations (cuda int32 tensors, one per level)."""
+        torch = _torch()
+        perms = []
+        for l in range(self.n_levels):
+            n = int(self.inp.n_points[l])
+            if n == 0:
+                perms.append(None)
+                continue
+            dev = torch.device("cuda", torch.cuda.current_device())
+            row = self.channels[l] * (4 if self.dtype == "f32" else 2)
+            pts = torch.empty(n * 16, dtype=torch.uint8, device=dev)
+            ref = torch.empty(n * row, dtype=torch.uint8, device=dev)
+            perm = torch.empty(n, dtype=torch.int32, device=dev)
+            tb = lib().pilot_refine_sort_anchors_temp_bytes(n)
+            tmp = torch.empty(tb + 256, dtype=torch.uint8, device=dev)
+            tptr = (tmp.data_ptr() + 255) // 256 * 256
+            st = stream if stream is not None else torch.cuda.current_stream()
+            _check(lib().pilot_refine_sort_anchors(self.inp.points_dev[l], self.inp.ref_feat_dev[l], n, self.channels[l],
+                                                   DTYPE_CODE[self.dtype], pts.data_ptr(), ref.data_ptr(), perm.data_ptr(),
+                                                   tptr, tb, C.c_void_p(st.cuda_stream)), "pilot_refine_sort_anchors")
+            st.synchronize()                      # tmp may go; the sorted buffers are kept alive by self.keep
+            self.keep += [pts, ref]
+            self.inp.points_dev[l], self.inp.ref_feat_dev[l] = pts.data_ptr(), ref.data_ptr()
+            perms.append(perm)
+        return perms
 
 
 class Refiner:

@@ -166,7 +166,7 @@ def test_paper_schedule_1210_to_128():
     # coarse objective of the kept hypotheses the two sides share
     common = [i for i, m in enumerate(g["kept_idx"]) if m in set(keep.tolist())]
     rel = np.abs(g["coarse_kept_cost"][common] - c0["cost64"][g["kept_idx"][common]]) / c0["cost64"][g["kept_idx"][common]]
-    assert np.median(rel) <= 5e-3 and (rel <= 5e-3).mean() >= 0.95, (np.median(rel), (rel <= 5e-3).mean())
+    assert rel.max() <= 5e-3, (rel.max(), g["kept_idx"][common][rel > 5e-3])      # every shared kept hypothesis (measured: 1.5e-5)
     assert np.all(np.diff(g["coarse_kept_cost"]) >= 0)                      # ascending order
     # the selected pose and objective
     assert parity.rot_angle(g["best_pose"], c1["poses64"][b])[0] <= 5e-3

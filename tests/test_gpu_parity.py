@@ -189,28 +189,40 @@ def test_host_path_matches_device_path():
     r.close()
 
 
-@pytest.mark.parametrize("name,stride", [("config2", 128), ("config4", 64)])
+@pytest.mark.parametrize("name,stride", [("config2", 64), ("config4", 16)])
 def test_full_size_sampled_hypotheses(name, stride):
-    """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle computes a strided
-    sample of hypotheses one by one (hypotheses are independent, so the sample is exact for those rows)."""
+    """BASELINE.json's full sizes in the launch configuration bench.py times (the tensor-core contraction under
+    math = mma, FFMA2 under -fp32); the oracle computes a strided sample of 16 hypotheses one by one (hypotheses are
+    independent, so the sample is exact for those rows). Free-running: the systems of record 0, the final poses of the
+    converged ones. Teacher-forced: the systems at the ORACLE's own iterates of records 3 and 7 (late iterates, where
+    the hypotheses have moved off their initial poses), full N, on the same kernel."""
     from oracle import pilot_oracle as po
     from paper_2606_31098_b200 import binding
     if MODE["mode"] not in ("passes", "split"):
         pytest.skip("full sizes run in bench.py's launch configuration (AUTO = one launch per pass at these sizes)")
     prob = wl.make(name)
-    gpu = binding.refine(prob, math=MODE["math"])
-    orc = po.run(po.Bound(prob), hyp_begin=0, hyp_step=stride, n_threads=8)
+    gpu = binding.refine(prob, mode=MODE["mode"], math=MODE["math"])
+    orc = po.run(po.Bound(prob), hyp_begin=0, hyp_step=stride, n_threads=16)
     idx = np.arange(0, prob["init_poses"].shape[0], stride)
+    assert len(idx) == 16
     g = {k: (v[:, idx] if k.startswith("iter_") else v[idx]) for k, v in gpu.items() if isinstance(v, np.ndarray)}
     o = {k: (v[:, idx] if k.startswith("iter_") else v[idx]) for k, v in orc.items() if isinstance(v, np.ndarray)}
     check_systems(g, o, "bf16", recs=(0,))
     # at these scene scales (ranges of 200-900 m) the last accepted steps are ~1e-5..1e-4 m: well inside the
     # 5e-3 pose tolerance, so 'converged' means last accepted |dxi| < 5e-4 here
     conv = parity.converged(o, step_tol=5e-4)
-    assert conv.sum() >= max(1, len(idx) // 2), conv.sum()
+    assert conv.sum() >= 12, conv.sum()                                   # at least 75 % of the sample
     er, et = parity.pose_errors(g, o)
     assert er[conv].max() <= 5e-3 and et[conv].max() <= 5e-3, (er[conv].max(), et[conv].max())
     assert np.abs(g["n_valid"][conv] - o["n_valid"][conv]).max() <= 2
+    # teacher-forced at the oracle's iterates: record k of the oracle = the system built at iter_poses[k]
+    for rec in (3, 7):
+        tf = parity.level_slice(prob, 0, o["iter_poses"][rec], iters=1)
+        gt = binding.refine(tf, mode=MODE["mode"], math=MODE["math"])
+        want = {"iter_hessian": o["iter_hessian"][rec:rec + 1], "iter_gradient": o["iter_gradient"][rec:rec + 1],
+                "iter_cost": o["iter_cost"][rec:rec + 1], "iter_gabs": o["iter_gabs"][rec:rec + 1]}
+        eH, eg, ec = parity.system_errors(gt, want, 0)
+        assert eH.max() <= 5e-3 and eg.max() <= 5e-3 and ec.max() <= 5e-3, (rec, eH.max(), eg.max(), ec.max())
     # properties that hold at any size: finite best cost, orthonormal rotations, cost never above the initial one
     R = gpu["poses"].reshape(-1, 3, 4)[:, :, :3]
     assert np.allclose(np.einsum("nij,nkj->nik", R, R), np.eye(3), atol=1e-5)
