@@ -43,7 +43,7 @@ extern "C" {
 #define PILOT_ERR_CUDA        (-4)  /* a CUDA runtime call failed                            */
 
 /* per-hypothesis status bits (outputs.status_dev) */
-#define PILOT_STATUS_NONFINITE   1u /* sticky: a non-finite cost / step was seen             */
+#define PILOT_STATUS_NONFINITE   1u /* sticky: a NaN total cost was seen (a non-finite STEP counts as a failed factorisation: bit 4) */
 #define PILOT_STATUS_FEW_VALID   2u /* the final accepted state has n_valid < min_valid (its cost is +inf) */
 #define PILOT_STATUS_CHOL_FAIL   4u /* sticky: Cholesky failed with lambda already at lambda_max */
 #define PILOT_STATUS_RANGE_SKIP  8u /* the final accepted state's range prior was skipped (ray leaves the DSM / no hit) */
@@ -171,12 +171,33 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in_
  * in host memory. Submitting run k+1 before waiting for run k overlaps its upload with run k's kernels. At most two
  * runs may be in flight (a third submit returns PILOT_ERR_UNSUPPORTED); the host buffers of a run (inputs: pinned
  * memory, or the upload serialises; outputs) must stay valid until its wait_host() returned.
- * run_host == submit_host + wait_host.
+ * run_host == submit_host + wait_host. The two runs in flight share the handle's workspace, so they execute one after the
+ * other: a run submitted on a different stream than the previous one is ordered behind it with an event. For every other
+ * entry point the rule is the usual one: calls on ONE handle (run, run_levels, sequence_step, ...) must be issued on one
+ * stream or be ordered by the caller; different handles are independent.
  */
 int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in_host,
                              const pilot_refine_params* p, const pilot_refine_outputs* out_host,
                              void* cuda_stream);
 int pilot_refine_wait_host(pilot_refine_handle* h);
+
+/*
+ * The paper's per-frame schedule (supp II-C PAPER.md:381-386, selection PAPER.md:168) through host buffers, one call per
+ * frame: upload of the frame's inputs (as submit_host: copy stream, two staging halves), then on `cuda_stream` the seeding
+ * of the n grid hypotheses around prior_pose_host ([12] row-major [R_wc | C]; pilot_refine_seed_hypotheses with the offsets
+ * of set_grid_host and `seed_frame`), the coarse level for all of them (run_levels 0..1), the `keep` lowest objectives
+ * (prune_topk), the finer levels for those (run_levels 1..n_levels), the arg-min (select_best), and the copy of the selected
+ * pose [12], its objective and its index INTO THE GRID to the three host pointers (each may be NULL). Returns a ticket;
+ * pilot_refine_wait_host() blocks until the oldest submitted frame's results are in host memory, so frame k+1 uploads while
+ * frame k refines. in_host->init_poses_dev and n_hypotheses are ignored. The handle comes from create_host with
+ * max_hypotheses >= n; set_grid_host copies the [n][6] offset table (pilot_refine_grid_offsets) to the device once (it
+ * allocates; not while runs are in flight; n <= PILOT_TOPK_MAX). Errors as submit_host; PILOT_ERR_ARG without a grid,
+ * for keep outside [1, n] or a one-level pyramid.
+ */
+int pilot_refine_set_grid_host(pilot_refine_handle* h, const float* offsets_host, int n);
+int pilot_refine_submit_pruned_host(pilot_refine_handle* h, const pilot_refine_inputs* in_host, const pilot_refine_params* p,
+                                    const float* prior_pose_host, int keep, int seed_frame, float* best_pose_host,
+                                    float* best_cost_host, int* best_index_host, void* cuda_stream);
 
 /*
  * Tuning knob: anchors per CTA of the photo kernel (a multiple of 128; 0 = built-in heuristic,

@@ -20,7 +20,7 @@
 #define PILOT_ERR_CUDA        (-4)  /* a CUDA runtime call failed                            */
 
 /* per-hypothesis status bits (outputs.status_dev) */
-#define PILOT_STATUS_NONFINITE   1u /* sticky: a non-finite cost / step was seen             */
+#define PILOT_STATUS_NONFINITE   1u /* sticky: a NaN total cost was seen (a non-finite STEP counts as a failed factorisation: bit 4) */
 #define PILOT_STATUS_FEW_VALID   2u /* the final accepted state has n_valid < min_valid (its cost is +inf) */
 #define PILOT_STATUS_CHOL_FAIL   4u /* sticky: Cholesky failed with lambda already at lambda_max */
 #define PILOT_STATUS_RANGE_SKIP  8u /* the final accepted state's range prior was skipped (ray leaves the DSM / no hit) */

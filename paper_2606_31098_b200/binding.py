@@ -35,6 +35,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
            "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
            "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
+           "pilot_refine_set_grid_host", "pilot_refine_submit_pruned_host",
            "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
@@ -178,6 +179,11 @@ def lib():
         L.pilot_refine_sort_anchors.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                 C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.pilot_refine_sort_anchors.restype = C.c_int
+        L.pilot_refine_set_grid_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.pilot_refine_set_grid_host.restype = C.c_int
+        L.pilot_refine_submit_pruned_host.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.c_void_p, C.c_int,
+                                                      C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_submit_pruned_host.restype = C.c_int
         for name in EXPORTS:
             if name.startswith("pilot_refine_sequence_"):
                 getattr(L, name).restype = C.c_int
@@ -700,6 +706,52 @@ class PrunedRefiner:
             self.visible_evals = vis
         return dict(best_idx=idx, best_pose=pose, best_cost=bc, kept_idx=kept_idx, poses=o1["poses"], cost=o1["cost"],
                     n_valid=o1["n_valid"], status=o1["status"], coarse_kept_cost=coarse_kept)
+
+    def close(self):
+        self.ref.close()
+
+
+class PrunedHostRefiner:
+    """The same schedule through HOST buffers, one C call per frame (pilot_refine_submit_pruned_host / _wait_host): frame
+    k+1 uploads while frame k refines. `hi` = DeviceInputs(prob, host=True) (pinned host tensors)."""
+
+    def __init__(self, hi, params, offsets, keep, seed_frame="world", device=0):
+        torch = _torch()
+        self.torch, self.device, self.hi, self.keep = torch, device, hi, int(keep)
+        off = np.ascontiguousarray(offsets, np.float32).reshape(-1, 6)
+        self.H0, self.frame = off.shape[0], SEED_CODE[seed_frame]
+        P = dict(DEFAULT_PARAMS); P.update(params or {})
+        self.par, _ = make_params(params, hi.n_levels)
+        dsm = (int(hi.inp.dsm_width), int(hi.inp.dsm_height))
+        self.ref = Refiner(hi.n_levels, hi.width, hi.height, hi.channels, hi.dtype, self.H0, max(1, hi.max_points),
+                           sum(P["iters"]), device=device, host_path=True, max_dsm=dsm)
+        _check(lib().pilot_refine_set_grid_host(self.ref.handle, off.ctypes.data, self.H0), "pilot_refine_set_grid_host")
+        self.res = [dict(pose=torch.zeros(12, dtype=torch.float32).pin_memory(), cost=torch.zeros(1, dtype=torch.float32).pin_memory(),
+                         index=torch.zeros(1, dtype=torch.int32).pin_memory()) for _ in range(2)]
+        self.priors = [torch.zeros(12, dtype=torch.float32).pin_memory() for _ in range(2)]
+        self.n_sub, self.pending = 0, []
+
+    def submit(self, prior_pose, stream=None):
+        k = self.n_sub & 1
+        self.priors[k].copy_(self.torch.as_tensor(np.asarray(prior_pose, np.float32).reshape(12)))
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        r = self.res[k]
+        t = lib().pilot_refine_submit_pruned_host(self.ref.handle, C.byref(self.hi.inp), C.byref(self.par), self.priors[k].data_ptr(),
+                                                  self.keep, self.frame, r["pose"].data_ptr(), r["cost"].data_ptr(),
+                                                  r["index"].data_ptr(), C.c_void_p(st.cuda_stream))
+        if t < 0:
+            _check(t, "pilot_refine_submit_pruned_host")
+        self.pending.append(k)
+        self.n_sub += 1
+        return t
+
+    def wait(self):
+        _check(lib().pilot_refine_wait_host(self.ref.handle), "pilot_refine_wait_host")
+        return self.res[self.pending.pop(0)]
+
+    @property
+    def launches(self):
+        return self.ref.last_launches
 
     def close(self):
         self.ref.close()

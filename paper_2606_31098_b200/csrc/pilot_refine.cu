@@ -98,6 +98,9 @@ struct pilot_refine_handle {
   cudaStream_t copy_stream; // uploads of submit_host
   cudaEvent_t ev_copied[2], ev_done[2];
   long n_submitted, n_waited;
+  // pruned host path (set_grid_host): one cudaMalloc
+  float* grid;              // offsets [n][6] | seeds [n][12] | two halves of GridHalf floats
+  int grid_n;
 };
 
 namespace {
@@ -263,6 +266,7 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->last_mma_levels = h->last_resident_levels = 0u;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
   h->copy_stream = nullptr; h->n_submitted = h->n_waited = 0;
+  h->grid = nullptr; h->grid_n = 0;
   for (int i = 0; i < 2; ++i) { h->ev_copied[i] = nullptr; h->ev_done[i] = nullptr; }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) { delete h; cudaSetDevice(prev); return PILOT_ERR_CUDA; }
@@ -296,6 +300,7 @@ int pilot_refine_destroy(pilot_refine_handle* h) {
     if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
   }
   if (h->stage) cudaFree(h->stage);
+  if (h->grid) cudaFree(h->grid);
   cudaSetDevice(prev);
   delete h;
   return PILOT_OK;
@@ -536,9 +541,15 @@ int pilot_refine_create_host(const pilot_refine_config* cfg, int max_dsm_width, 
   return PILOT_OK;
 }
 
-int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
-                             const pilot_refine_outputs* out, void* cuda_stream) {
-  if (!h || !in || !p || !out || !h->host_mode) return PILOT_ERR_ARG;
+}  // extern "C"
+
+namespace {
+
+// Checks of a host-path submission and the upload of every input of `in` (host pointers) into staging half `half` on the
+// handle's copy stream; `din` = the same inputs with device pointers. The compute stream waits for the upload (and for the
+// previous run, which shares the workspace). Returns PILOT_OK or an error; T = sum of iterations.
+int host_upload(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p, cudaStream_t st, int half,
+                pilot_refine_inputs* din, int* T_out) {
   const pilot_refine_config& c = h->cfg;
   if (in->n_hypotheses < 0 || in->n_hypotheses > c.max_hypotheses) return in->n_hypotheses < 0 ? PILOT_ERR_ARG : PILOT_ERR_UNSUPPORTED;
   int T = 0;
@@ -550,15 +561,10 @@ int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* 
   if (T > c.max_total_iters) return PILOT_ERR_UNSUPPORTED;
   if (in->dsm_dev && ((size_t)in->dsm_width * in->dsm_height > (size_t)h->max_dsm_w * h->max_dsm_h)) return PILOT_ERR_UNSUPPORTED;
   if (h->n_submitted - h->n_waited >= 2) return PILOT_ERR_UNSUPPORTED;      // both halves in flight
-  int prev = 0;
-  cudaGetDevice(&prev);
-  if (prev != c.device && cudaSetDevice(c.device) != cudaSuccess) return PILOT_ERR_CUDA;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  const int half = (int)(h->n_submitted & 1);
   char* stage = h->stage + (size_t)half * h->stage_bytes;
   StageLayout s = stage_layout(&c, h->max_dsm_w, h->max_dsm_h);
   size_t es = elem_size(c.feat_dtype), H = (size_t)in->n_hypotheses;
-  pilot_refine_inputs din = *in;
+  *din = *in;
   bool ok = true;
   // the run that last used this half (two submissions ago) has been waited for, so the half is free on the device
   auto up = [&](size_t at, const void* src, size_t bytes) -> void* {
@@ -568,15 +574,60 @@ int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* 
   };
   for (int l = 0; l < c.n_levels; ++l) {
     size_t px = (size_t)c.width[l] * c.height[l], N = (size_t)in->n_points[l];
-    din.query_feat_dev[l] = up(s.feat[l], in->query_feat_dev[l], px * c.channels[l] * es);
-    din.query_conf_dev[l] = static_cast<const float*>(up(s.conf[l], in->query_conf_dev[l], px * 4));
-    din.points_dev[l] = static_cast<const float*>(up(s.pts[l], in->points_dev[l], N * 16));
-    din.ref_feat_dev[l] = up(s.ref[l], in->ref_feat_dev[l], N * c.channels[l] * es);
+    din->query_feat_dev[l] = up(s.feat[l], in->query_feat_dev[l], px * c.channels[l] * es);
+    din->query_conf_dev[l] = static_cast<const float*>(up(s.conf[l], in->query_conf_dev[l], px * 4));
+    din->points_dev[l] = static_cast<const float*>(up(s.pts[l], in->points_dev[l], N * 16));
+    din->ref_feat_dev[l] = up(s.ref[l], in->ref_feat_dev[l], N * c.channels[l] * es);
   }
-  din.init_poses_dev = static_cast<const float*>(up(s.poses, in->init_poses_dev, H * 48));
-  din.dsm_dev = static_cast<const float*>(up(s.dsm, in->dsm_dev, (size_t)in->dsm_width * in->dsm_height * 4));
+  din->init_poses_dev = static_cast<const float*>(up(s.poses, in->init_poses_dev, H * 48));
+  din->dsm_dev = static_cast<const float*>(up(s.dsm, in->dsm_dev, (size_t)in->dsm_width * in->dsm_height * 4));
   ok = ok && cudaEventRecord(h->ev_copied[half], h->copy_stream) == cudaSuccess;
   ok = ok && cudaStreamWaitEvent(st, h->ev_copied[half], 0) == cudaSuccess;
+  // both runs in flight share the handle's workspace (optimiser state, partial sums): if the previous run was submitted on
+  // ANOTHER stream, this run's kernels must still come after it (a no-op when the caller keeps to one stream)
+  if (h->n_submitted > h->n_waited) ok = ok && cudaStreamWaitEvent(st, h->ev_done[half ^ 1], 0) == cudaSuccess;
+  *T_out = T;
+  return ok ? PILOT_OK : PILOT_ERR_CUDA;
+}
+
+// floats of one half of the pruned path's device block
+struct GridHalf { size_t prior, kept_idx, kept_poses, kept_cost, best, total; };
+GridHalf grid_half(int n) {
+  GridHalf g;
+  size_t o = 0;
+  g.prior = o; o += 16;
+  g.kept_idx = o; o += (size_t)(n + 3) / 4 * 4;
+  g.kept_poses = o; o += (size_t)n * 12;
+  g.kept_cost = o; o += (size_t)(n + 3) / 4 * 4;
+  g.best = o; o += 16;                       // best_idx (in the kept set) | grid index | best_cost | pad | best_pose[12]
+  o += 16;
+  g.total = o;
+  return g;
+}
+
+__global__ void best_grid_index_kernel(const int* kept_idx, const int* best_idx, int* out) { *out = kept_idx[*best_idx]; }
+
+}  // namespace
+
+extern "C" {
+
+int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                             const pilot_refine_outputs* out, void* cuda_stream) {
+  if (!h || !in || !p || !out || !h->host_mode) return PILOT_ERR_ARG;
+  const pilot_refine_config& c = h->cfg;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != c.device && cudaSetDevice(c.device) != cudaSuccess) return PILOT_ERR_CUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int half = (int)(h->n_submitted & 1);
+  char* stage = h->stage + (size_t)half * h->stage_bytes;
+  StageLayout s = stage_layout(&c, h->max_dsm_w, h->max_dsm_h);
+  pilot_refine_inputs din;
+  int T = 0;
+  int rc = host_upload(h, in, p, st, half, &din, &T);
+  if (rc != PILOT_OK) { if (prev != c.device) cudaSetDevice(prev); return rc; }
+  const size_t H = (size_t)in->n_hypotheses;
+  bool ok = true;
   pilot_refine_outputs dout;
   dout.poses_dev = out->poses_dev ? reinterpret_cast<float*>(stage + s.o_poses) : nullptr;
   dout.cost_dev = out->cost_dev ? reinterpret_cast<float*>(stage + s.o_cost) : nullptr;
@@ -586,7 +637,7 @@ int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* 
   dout.iter_gradient_dev = out->iter_gradient_dev ? reinterpret_cast<float*>(stage + s.o_ig) : nullptr;
   dout.iter_cost_dev = out->iter_cost_dev ? reinterpret_cast<float*>(stage + s.o_ic) : nullptr;
   dout.iter_lambda_dev = out->iter_lambda_dev ? reinterpret_cast<float*>(stage + s.o_il) : nullptr;
-  int rc = ok ? pilot_refine_run(h, &din, p, &dout, cuda_stream) : PILOT_ERR_CUDA;
+  rc = pilot_refine_run(h, &din, p, &dout, cuda_stream);
   if (rc == PILOT_OK) {
     auto down = [&](void* dst, const void* src, size_t bytes) {
       if (dst && bytes) ok = ok && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
@@ -602,6 +653,91 @@ int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* 
     ok = ok && cudaEventRecord(h->ev_done[half], st) == cudaSuccess;
     if (!ok) rc = PILOT_ERR_CUDA;
   }
+  if (prev != c.device) cudaSetDevice(prev);
+  if (rc != PILOT_OK) return rc;
+  const int ticket = (int)(h->n_submitted & 0x3fffffff);
+  h->n_submitted += 1;
+  return ticket;
+}
+
+int pilot_refine_set_grid_host(pilot_refine_handle* h, const float* offsets_host, int n) {
+  if (!h || !h->host_mode || !offsets_host || n < 1) return PILOT_ERR_ARG;
+  if (n > h->cfg.max_hypotheses || n > PILOT_TOPK_MAX) return PILOT_ERR_UNSUPPORTED;
+  if (h->n_submitted != h->n_waited) return PILOT_ERR_ARG;                  // not while runs are in flight
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != h->cfg.device && cudaSetDevice(h->cfg.device) != cudaSuccess) return PILOT_ERR_CUDA;
+  if (h->grid) { cudaFree(h->grid); h->grid = nullptr; h->grid_n = 0; }
+  const size_t floats = (size_t)n * 18 + 2 * grid_half(n).total;
+  void* g = nullptr;
+  bool ok = cudaMalloc(&g, floats * sizeof(float)) == cudaSuccess &&
+            cudaMemcpy(g, offsets_host, (size_t)n * 6 * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess;
+  if (ok) { h->grid = static_cast<float*>(g); h->grid_n = n; } else if (g) cudaFree(g);
+  if (prev != h->cfg.device) cudaSetDevice(prev);
+  return ok ? PILOT_OK : PILOT_ERR_CUDA;
+}
+
+int pilot_refine_submit_pruned_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                                    const float* prior_pose_host, int keep, int seed_frame, float* best_pose_host,
+                                    float* best_cost_host, int* best_index_host, void* cuda_stream) {
+  if (!h || !in || !p || !prior_pose_host || !h->host_mode || !h->grid) return PILOT_ERR_ARG;
+  const pilot_refine_config& c = h->cfg;
+  const int n = h->grid_n;
+  if (keep < 1 || keep > n || c.n_levels < 2) return PILOT_ERR_ARG;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != c.device && cudaSetDevice(c.device) != cudaSuccess) return PILOT_ERR_CUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const int half = (int)(h->n_submitted & 1);
+  char* stage = h->stage + (size_t)half * h->stage_bytes;
+  StageLayout s = stage_layout(&c, h->max_dsm_w, h->max_dsm_h);
+  pilot_refine_inputs hin = *in, din;
+  hin.n_hypotheses = n;
+  hin.init_poses_dev = nullptr;                                            // the seeds are made on the device
+  int T = 0;
+  int rc = host_upload(h, &hin, p, st, half, &din, &T);
+  if (rc != PILOT_OK) { if (prev != c.device) cudaSetDevice(prev); return rc; }
+  const GridHalf G = grid_half(n);
+  float* offsets = h->grid;
+  float* seeds = h->grid + (size_t)n * 6;
+  float* gh = h->grid + (size_t)n * 18 + (size_t)half * G.total;
+  float* prior = gh + G.prior;
+  int* kept_idx = reinterpret_cast<int*>(gh + G.kept_idx);
+  float *kept_poses = gh + G.kept_poses, *kept_cost = gh + G.kept_cost;
+  int* best_idx = reinterpret_cast<int*>(gh + G.best);
+  int* best_grid = best_idx + 1;
+  float* best_cost = gh + G.best + 2;
+  float* best_pose = gh + G.best + 4;
+  // the prior (48 bytes) is copied on the compute stream: the upload event of this half is already recorded
+  bool ok = cudaMemcpyAsync(prior, prior_pose_host, 48, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  pilot_refine_outputs dout;
+  memset(&dout, 0, sizeof dout);
+  dout.poses_dev = reinterpret_cast<float*>(stage + s.o_poses);
+  dout.cost_dev = reinterpret_cast<float*>(stage + s.o_cost);
+  int launches = 0;
+  if (ok) rc = pilot_refine_seed_hypotheses(prior, offsets, n, seed_frame, seeds, cuda_stream);
+  if (ok && rc == PILOT_OK) {
+    din.n_hypotheses = n; din.init_poses_dev = seeds;
+    rc = pilot_refine_run_levels(h, &din, p, &dout, 0, 1, cuda_stream);                       // coarse level, all hypotheses
+    launches += h->last_launches + 1;
+  }
+  if (ok && rc == PILOT_OK) rc = pilot_refine_prune_topk(dout.cost_dev, dout.poses_dev, n, keep, kept_idx, kept_poses, kept_cost, cuda_stream);
+  if (ok && rc == PILOT_OK) {
+    din.n_hypotheses = keep; din.init_poses_dev = kept_poses;
+    rc = pilot_refine_run_levels(h, &din, p, &dout, 1, c.n_levels, cuda_stream);              // finer levels, the kept ones
+    launches += h->last_launches + 1;
+  }
+  if (ok && rc == PILOT_OK) rc = pilot_refine_select_best(dout.cost_dev, dout.poses_dev, keep, best_idx, best_pose, best_cost, cuda_stream);
+  if (ok && rc == PILOT_OK) {
+    best_grid_index_kernel<<<1, 1, 0, st>>>(kept_idx, best_idx, best_grid);
+    launches += 2;
+    if (best_pose_host) ok = ok && cudaMemcpyAsync(best_pose_host, best_pose, 48, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+    if (best_cost_host) ok = ok && cudaMemcpyAsync(best_cost_host, best_cost, 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+    if (best_index_host) ok = ok && cudaMemcpyAsync(best_index_host, best_grid, 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+    ok = ok && cudaEventRecord(h->ev_done[half], st) == cudaSuccess;
+  }
+  h->last_launches = launches;
+  if (!ok && rc == PILOT_OK) rc = PILOT_ERR_CUDA;
   if (prev != c.device) cudaSetDevice(prev);
   if (rc != PILOT_OK) return rc;
   const int ticket = (int)(h->n_submitted & 0x3fffffff);

@@ -176,3 +176,37 @@ def test_paper_schedule_1210_to_128():
     # and it is a localisation: the 3.1 m / -4.3 m / 2.2 deg prior error is removed
     gt = prob["gt_pose"]
     assert np.rad2deg(parity.rot_angle(g["best_pose"], gt))[0] < 0.1 and parity.trans_dist(g["best_pose"], gt)[0] < 0.3
+
+
+def test_pruned_host_path_matches_the_device_path():
+    """pilot_refine_submit_pruned_host (one call per frame through host buffers, two frames in flight) gives the same
+    selection, bit for bit, as the five device calls of PrunedRefiner (same kernels, same order)."""
+    import torch
+    from paper_2606_31098_b200 import binding, workloads as wl
+    prob = wl.paper_frame()
+    xy_range, xy_step, yaws = prob["grid"]
+    off = binding.grid_offsets(xy_range, xy_step, yaws, -np.asarray(prob["gravity_world"], np.float64))
+    di = binding.DeviceInputs(prob)
+    pr = binding.PrunedRefiner(di, prob["params"], off, prob["keep"], "world")
+    out = pr.run(dev(prob["prior_pose"]))
+    torch.cuda.synchronize()
+    want_pose, want_cost = out["best_pose"].cpu().numpy(), out["best_cost"].cpu().numpy()
+    want_idx = int(out["kept_idx"].cpu().numpy()[int(out["best_idx"].cpu().numpy()[0])])
+    pr.close()
+    hi = binding.DeviceInputs(prob, host=True)
+    ph = binding.PrunedHostRefiner(hi, prob["params"], off, prob["keep"], "world")
+    prior2 = prob["prior_pose"].copy(); prior2[3] += 0.7                      # a second frame with another prior, in flight too
+    ph.submit(prob["prior_pose"]); ph.submit(prior2)
+    r0 = {k: v.clone() for k, v in ph.wait().items()}
+    ph.submit(prob["prior_pose"])
+    r1 = {k: v.clone() for k, v in ph.wait().items()}
+    r2 = {k: v.clone() for k, v in ph.wait().items()}
+    for r in (r0, r2):
+        assert np.array_equal(r["pose"].numpy(), want_pose.reshape(-1)) and r["cost"].numpy()[0] == want_cost[0]
+        assert int(r["index"].numpy()[0]) == want_idx
+    assert not np.array_equal(r1["pose"].numpy(), want_pose.reshape(-1))      # the other prior gave another answer
+    assert parity.trans_dist(r1["pose"].numpy(), prob["gt_pose"])[0] < 0.3    # ... which is still a localisation
+    with pytest.raises(RuntimeError):
+        ph.submit(prob["prior_pose"]); ph.submit(prob["prior_pose"]); ph.submit(prob["prior_pose"])   # third in flight
+    ph.wait(); ph.wait()
+    ph.close()
