@@ -81,3 +81,110 @@ def test_visible_set_and_empty_set():
     far = np.hstack([np.eye(3), np.array([[0.0], [0.0], [200.0]])]).reshape(12)
     L, n = ps.reprojection_loss(far[None], pose, pts, K, 640, 480, 0.1, 1.0, 1.0)
     assert n[0] == 0
+
+
+# ------------------------------------------------------------------ backward pieces, pinned by central differences
+
+def _xi_mat(xi):
+    M = np.zeros((4, 4))
+    M[:3, :3] = [[0, -xi[5], xi[4]], [xi[5], 0, -xi[3]], [-xi[4], xi[3], 0]]
+    M[:3, 3] = xi[:3]
+    return M
+
+
+def _T_cw(pose):
+    T = np.asarray(pose, np.float64).reshape(3, 4)
+    M = np.eye(4); M[:3, :3] = T[:, :3].T; M[:3, 3] = -T[:, :3].T @ T[:, 3]
+    return M
+
+
+def _pose_of(M):
+    R_wc = M[:3, :3].T
+    return np.concatenate([R_wc, (-R_wc @ M[:3, 3])[:, None]], 1).reshape(-1)
+
+
+def _bscene(seed=5, n=300):
+    rng = np.random.default_rng(seed)
+    pts = np.concatenate([rng.uniform(-40, 40, (n, 2)), rng.uniform(0, 10, (n, 1)), np.ones((n, 1))], 1)
+    from tests.small_problems import look_down_pose
+    Ts = look_down_pose(np.array([0.0, -60.0, 100.0])).reshape(-1)
+    K = (300.0, 310.0, 160.0, 120.0)
+    return pts, Ts, K
+
+
+def test_loss_gradient_matches_central_differences_of_the_forward_value():
+    from scipy.linalg import expm
+    pts, Ts, K = _bscene()
+    Tk = _pose_of(expm(_xi_mat(np.array([1.5, -2.0, 0.8, 0.02, -0.015, 0.03]))) @ _T_cw(Ts))
+    for alpha, c in [(2.0, 1.0), (1.0, 3.0), (0.0, 2.0), (-2.0, 4.0), (-np.inf, 5.0), (0.5, 2.5)]:
+        L, n, G = ps.reprojection_loss_grad(Tk[None], Ts, pts, K, 320, 240, 0.1, alpha, c)
+        L0, n0 = ps.reprojection_loss(Tk[None], Ts, pts, K, 320, 240, 0.1, alpha, c)
+        assert L[0] == L0[0] and n[0] == n0[0] and n[0] > 100
+        for i in range(6):
+            e = np.zeros(6); e[i] = 1e-6
+            Lp = ps.reprojection_loss(_pose_of(expm(_xi_mat(e)) @ _T_cw(Tk))[None], Ts, pts, K, 320, 240, 0.1, alpha, c)[0][0]
+            Lm = ps.reprojection_loss(_pose_of(expm(_xi_mat(-e)) @ _T_cw(Tk))[None], Ts, pts, K, 320, 240, 0.1, alpha, c)[0][0]
+            assert (Lp - Lm) / 2e-6 == pytest.approx(G[0, i], rel=2e-6, abs=1e-9 * np.abs(G[0]).max()), (alpha, i)
+    # at the ground truth the loss is stationary
+    assert np.allclose(ps.reprojection_loss_grad(Ts[None], Ts, pts, K, 320, 240, 0.1, 1.0, 2.0)[2], 0.0, atol=1e-15)
+
+
+def test_left_jacobian_defining_property():
+    from scipy.linalg import expm, logm
+    rng = np.random.default_rng(8)
+    for scale in (1e-3, 0.2, 1.0):
+        xi = rng.normal(size=6) * scale
+        J = ps.se3_left_jacobian(xi)
+        for i in range(6):
+            d = np.zeros(6); d[i] = 1e-6
+            Lg = np.real(logm(expm(_xi_mat(xi + d)) @ np.linalg.inv(expm(_xi_mat(xi)))))     # exp((J_l d)^) to first order
+            col = np.array([Lg[0, 3], Lg[1, 3], Lg[2, 3], Lg[2, 1], Lg[0, 2], Lg[1, 0]]) / 1e-6
+            assert np.allclose(col, J[:, i], atol=5e-6 * max(1.0, scale))
+    assert np.allclose(ps.se3_left_jacobian(np.zeros(6)), np.eye(6))
+    xi = rng.normal(size=6) * 0.3
+    assert np.allclose(ps.se3_exp_matrix(xi), expm(_xi_mat(xi)), atol=1e-13)
+
+
+@pytest.mark.parametrize("diag", [False, True])
+def test_lm_step_adjoint_matches_central_differences_of_the_composed_map(diag):
+    """f(H, g, eps) = L(exp(dxi(H, g)^) exp(eps^) T^k): dL/dg, dL/dH (symmetric perturbations) and q_prev = df/d eps."""
+    from scipy.linalg import expm
+    pts, Ts, K = _bscene(seed=6)
+    rng = np.random.default_rng(11)
+    Tk = expm(_xi_mat(np.array([2.0, 1.0, -1.5, -0.02, 0.03, 0.01]))) @ _T_cw(Ts)
+    B = rng.normal(size=(12, 6)) * np.array([1, 1, 1, 30, 30, 30])
+    Hm = B.T @ B
+    g = rng.normal(size=6) * np.array([1.0, 1.0, 1.0, 40.0, 40.0, 40.0])
+    lam = 0.3 if diag else 5.0
+    al, c = 1.0, 3.0
+
+    def step(Hm, g):
+        D = np.diag(np.maximum(np.diag(Hm), 1e-12)) if diag else np.eye(6)
+        return -np.linalg.solve(Hm + lam * D, g)
+
+    def f(Hm, g, eps=np.zeros(6)):
+        T = expm(_xi_mat(step(Hm, g))) @ expm(_xi_mat(eps)) @ Tk
+        return ps.reprojection_loss(_pose_of(T)[None], Ts, pts, K, 320, 240, 0.1, al, c)[0][0]
+
+    dxi0 = step(Hm, g)
+    assert 0.05 < np.linalg.norm(dxi0[:3]) < 5 and np.linalg.norm(dxi0[3:]) > 1e-3      # a step large enough for J_l to matter
+    T1 = _pose_of(expm(_xi_mat(dxi0)) @ Tk)
+    q = ps.reprojection_loss_grad(T1[None], Ts, pts, K, 320, 240, 0.1, al, c)[2][0]
+    dxi, GH, Gg, qp = ps.lm_step_adjoint(Hm, g, lam, diag, q)
+    assert np.allclose(dxi, dxi0)
+    scale_g = np.abs(Gg).max()
+    for i in range(6):
+        h = 1e-5 * max(1.0, abs(g[i]))
+        e = np.zeros(6); e[i] = h
+        assert (f(Hm, g + e) - f(Hm, g - e)) / (2 * h) == pytest.approx(Gg[i], rel=1e-5, abs=1e-7 * scale_g)
+    scale_H = np.abs(GH).max()
+    for i in range(6):
+        for j in range(i, 6):
+            h = 1e-5 * max(1.0, abs(Hm[i, j]))
+            E = np.zeros((6, 6)); E[i, j] = E[j, i] = h
+            fd = (f(Hm + E, g) - f(Hm - E, g)) / (2 * h)
+            want = GH[i, j] if i == j else 2 * GH[i, j]            # dL = <G_H, dH>: an off-diagonal pair is perturbed together
+            assert fd == pytest.approx(want, rel=2e-5, abs=1e-6 * scale_H), (i, j)
+    for i in range(6):
+        e = np.zeros(6); e[i] = 1e-6
+        assert (f(Hm, g, e) - f(Hm, g, -e)) / 2e-6 == pytest.approx(qp[i], rel=1e-5, abs=1e-8 * np.abs(qp).max())
