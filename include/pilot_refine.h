@@ -428,6 +428,27 @@ int pilot_refine_reprojection_loss(const float* poses_dev, int n_poses, const fl
                                    int width, int height, float z_near, float alpha, float scale,
                                    float* loss_dev, int* n_visible_dev, void* cuda_stream);
 
+/*
+ * Backward pieces of the unrolled refinement ("the refinement is unrolled over nine coarse-to-fine steps",
+ * supp III-C PAPER.md:427-440). reprojection_loss_grad: as reprojection_loss, plus grad_dev[k][6] = dL_k / d eps for the left
+ * perturbation T_cw <- exp(eps^) T_cw of pose k (eps = (rho; phi), the LM's own parametrisation: reading A1/A2 of DESIGN.md);
+ * loss_dev / n_visible_dev may be NULL. lm_step_adjoint: for n independent LM steps dxi = -(H + lambda D)^-1 g (Eq.8,
+ * PAPER.md:160-164; D = I or diag(max(H_ii, 1e-12)) per damp_mode), T' = exp(dxi^) T (Eq.9), given q_dev[m][6] = dL / d eps
+ * at the UPDATED pose: dxi_dev[m][6]; grad_gradient_dev[m][6] = dL/dg; grad_hessian_dev[m][36] = dL/dH, symmetric, such that
+ * dL = <dL/dH, dH> for symmetric dH; q_prev_dev[m][6] (optional) = the part of dL / d eps at the PREVIOUS pose that flows
+ * through the retraction, Ad(exp(dxi^))^T q; status_dev[m] (optional) = PILOT_STATUS_CHOL_FAIL if H + lambda D is not
+ * positive definite. hessian_dev [n][36] row-major (symmetrised on read), gradient_dev [n][6], lambda_dev [n]: what
+ * pilot_refine_run records per iteration. Not built: the dependence of H and g on the pose and on the feature maps (the
+ * transpose of the gather). Asynchronous on cuda_stream; double arithmetic, one rounding to fp32 on output.
+ */
+int pilot_refine_reprojection_loss_grad(const float* poses_dev, int n_poses, const float pose_star[12],
+                                        const float* points_dev, int n_points, const float intrinsics[4],
+                                        int width, int height, float z_near, float alpha, float scale,
+                                        float* loss_dev, int* n_visible_dev, float* grad_dev, void* cuda_stream);
+int pilot_refine_lm_step_adjoint(const float* hessian_dev, const float* gradient_dev, const float* lambda_dev,
+                                 const float* q_dev, int n, int damp_mode, float* dxi_dev, float* grad_hessian_dev,
+                                 float* grad_gradient_dev, float* q_prev_dev, unsigned* status_dev, void* cuda_stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Anchor order (kernel description PAPER.md:485). The sums of Eq.(2) and Eq.(8) do not depend on the
  * order of the anchors, but the THROUGHPUT of pilot_refine_run does: CTAs that run together sweep the same batches of

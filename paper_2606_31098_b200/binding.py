@@ -36,6 +36,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
            "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
            "pilot_refine_set_grid_host", "pilot_refine_submit_pruned_host",
+           "pilot_refine_reprojection_loss_grad", "pilot_refine_lm_step_adjoint",
            "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
@@ -179,6 +180,13 @@ def lib():
         L.pilot_refine_sort_anchors.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
                                                 C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         L.pilot_refine_sort_anchors.restype = C.c_int
+        L.pilot_refine_reprojection_loss_grad.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_float), C.c_void_p, C.c_int,
+                                                          C.POINTER(C.c_float), C.c_int, C.c_int, C.c_float, C.c_float, C.c_float,
+                                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_reprojection_loss_grad.restype = C.c_int
+        L.pilot_refine_lm_step_adjoint.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p,
+                                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_lm_step_adjoint.restype = C.c_int
         L.pilot_refine_set_grid_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.pilot_refine_set_grid_host.restype = C.c_int
         L.pilot_refine_submit_pruned_host.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.c_void_p, C.c_int,
@@ -822,3 +830,37 @@ def reprojection_loss(poses, pose_star, points, intrinsics, width, height, z_nea
                                                 loss.data_ptr(), nvis.data_ptr(), _stream_ptr(torch, stream, poses.device)),
            "pilot_refine_reprojection_loss")
     return loss, nvis
+
+
+def reprojection_loss_grad(poses, pose_star, points, intrinsics, width, height, z_near, alpha, scale, stream=None):
+    """As reprojection_loss, plus dL/d eps [n, 6] for the left perturbation of T_cw (eps = (rho; phi))."""
+    torch = _torch()
+    assert poses.is_cuda and points.is_cuda and poses.dtype == points.dtype == torch.float32
+    n = int(poses.shape[0])
+    K = (C.c_float * 4)(*[float(k) for k in intrinsics])
+    Ts = (C.c_float * 12)(*[float(t) for t in pose_star])
+    loss = torch.empty(n, dtype=torch.float32, device=poses.device)
+    nvis = torch.empty(n, dtype=torch.int32, device=poses.device)
+    grad = torch.empty(n, 6, dtype=torch.float32, device=poses.device)
+    _check(lib().pilot_refine_reprojection_loss_grad(poses.data_ptr(), n, Ts, points.data_ptr(), int(points.shape[0]), K,
+                                                     int(width), int(height), float(z_near), float(alpha), float(scale),
+                                                     loss.data_ptr(), nvis.data_ptr(), grad.data_ptr(),
+                                                     _stream_ptr(torch, stream, poses.device)), "pilot_refine_reprojection_loss_grad")
+    return loss, nvis, grad
+
+
+def lm_step_adjoint(hessian, gradient, lam, q, damp="identity", stream=None):
+    """Adjoint of n LM steps. hessian [n, 36], gradient [n, 6], lam [n], q [n, 6] (cuda float32).
+    -> dict(dxi, grad_hessian [n, 36], grad_gradient, q_prev, status)."""
+    torch = _torch()
+    n = int(hessian.shape[0])
+    dev = hessian.device
+    o = dict(dxi=torch.empty(n, 6, dtype=torch.float32, device=dev), grad_hessian=torch.empty(n, 36, dtype=torch.float32, device=dev),
+             grad_gradient=torch.empty(n, 6, dtype=torch.float32, device=dev), q_prev=torch.empty(n, 6, dtype=torch.float32, device=dev),
+             status=torch.empty(n, dtype=torch.int32, device=dev))
+    _check(lib().pilot_refine_lm_step_adjoint(hessian.contiguous().data_ptr(), gradient.contiguous().data_ptr(),
+                                              lam.contiguous().data_ptr(), q.contiguous().data_ptr(), n, DAMP_CODE[damp],
+                                              o["dxi"].data_ptr(), o["grad_hessian"].data_ptr(), o["grad_gradient"].data_ptr(),
+                                              o["q_prev"].data_ptr(), o["status"].data_ptr(), _stream_ptr(torch, stream, dev)),
+           "pilot_refine_lm_step_adjoint")
+    return o

@@ -79,3 +79,46 @@ def test_supervision_of_an_unrolled_refinement_decreases():
     Lo, no = ps.reprojection_loss(poses, Ts, pts, K, 64, 48, 0.1, 1.0, 1.0)
     assert np.array_equal(n.cpu().numpy(), no) and np.allclose(L.cpu().numpy(), Lo, rtol=2e-6, atol=1e-12)
     assert no[0] > 100 and Lo[0] > 0.1 and Lo[-1] < 0.05 * Lo[0]
+
+
+def test_backward_pieces_match_the_oracle():
+    """Pose gradient of the reprojection loss and the adjoint of LM steps taken from a real run's records (config 0),
+    against oracle/pilot_supervision.py (itself pinned by central differences): double arithmetic on both sides, one
+    rounding to fp32 on the GPU's outputs."""
+    import torch
+    from oracle import pilot_oracle as po
+    from oracle import pilot_supervision as ps
+    from paper_2606_31098_b200 import binding, workloads as wl
+    prob = wl.config0()
+    orc = po.run(po.Bound(prob, dict(iters=[6])))
+    poses = np.concatenate([prob["init_poses"][:1], orc["iter_poses"][1:, 0].astype(np.float32), orc["poses"][:1]])
+    pts = prob["points"][0]
+    K, W, H = prob["intrinsics"][0], prob["width"][0], prob["height"][0]
+    d = torch.device("cuda")
+    for alpha, c in [(1.0, 2.0), (2.0, 1.0), (0.0, 3.0), (-2.0, 1.5), (-np.inf, 4.0)]:
+        L, nv, G = binding.reprojection_loss_grad(torch.from_numpy(poses).to(d), prob["gt_pose"], torch.from_numpy(pts).to(d), K, W, H,
+                                                  0.1, alpha, c)
+        Lo, no, Go = ps.reprojection_loss_grad(poses, np.asarray(prob["gt_pose"], np.float32), pts, K, W, H, 0.1, alpha, c)
+        assert np.array_equal(nv.cpu().numpy(), no) and no.min() > 50
+        assert np.allclose(L.cpu().numpy(), Lo, rtol=2e-6, atol=1e-12)
+        assert np.allclose(G.cpu().numpy(), Go, rtol=2e-6, atol=2e-6 * np.abs(Go).max())
+    # the recorded systems of the run, the gradient of L at the pose each step produced
+    Hs, gs, lam = orc["iter_hessian"][:, 0], orc["iter_gradient"][:, 0], orc["iter_lambda"][:, 0]
+    nxt = np.concatenate([orc["iter_poses"][1:, 0], orc["poses64"][:1]]).astype(np.float32)
+    q = ps.reprojection_loss_grad(nxt, np.asarray(prob["gt_pose"], np.float32), pts, K, W, H, 0.1, 1.0, 2.0)[2].astype(np.float32)
+    for damp in ("identity", "diag"):
+        o = binding.lm_step_adjoint(torch.from_numpy(Hs).to(d), torch.from_numpy(gs).to(d), torch.from_numpy(lam).to(d),
+                                    torch.from_numpy(q).to(d), damp)
+        o = {k: v.cpu().numpy() for k, v in o.items()}
+        assert np.all(o["status"] == 0)
+        for m in range(Hs.shape[0]):
+            dxi, GH, Gg, qp = ps.lm_step_adjoint(Hs[m].astype(np.float64), gs[m].astype(np.float64), float(lam[m]), damp == "diag",
+                                                 q[m].astype(np.float64))
+            assert np.allclose(o["dxi"][m], dxi, rtol=1e-5, atol=1e-6 * np.abs(dxi).max())
+            assert np.allclose(o["grad_gradient"][m], Gg, rtol=1e-5, atol=1e-6 * np.abs(Gg).max())
+            assert np.allclose(o["grad_hessian"][m].reshape(6, 6), GH, rtol=1e-5, atol=1e-6 * np.abs(GH).max())
+            assert np.allclose(o["q_prev"][m], qp, rtol=1e-5, atol=1e-6 * np.abs(qp).max())
+    # a system that is not positive definite is flagged, not an error return
+    bad = binding.lm_step_adjoint(torch.from_numpy(-Hs[:1]).to(d), torch.from_numpy(gs[:1]).to(d), torch.zeros(1, device=d),
+                                  torch.from_numpy(q[:1]).to(d))
+    assert int(bad["status"].cpu().numpy()[0]) == 4
