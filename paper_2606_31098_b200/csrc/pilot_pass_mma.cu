@@ -1,16 +1,22 @@
 // pilot_pass_mma.cu — the pass kernel with the tensor-core contraction (pilot_math_mode MMA), in a translation unit of
-// its own because its CTA shape differs: 4 warps at 72 registers, 7 CTAs = 28 warps per SM. Once the contraction is on
-// the tensor cores the gather is bound by load latency and by the L1 data path (85 % busy), not by issue slots, and
-// warps hide that better than registers of prefetched taps; measured on config 4 (B200, ms per step): 16 warps per SM at
-// 128 registers with 6 rounds of 16-byte taps in flight 11.27; 32 warps at 64 registers with 2 rounds in flight 10.29;
-// 32-byte loads (LDG.256, half the rounds), 28 warps at 72 registers, 1 round in flight 9.60 (FFMA2 path: 11.89).
-// Shares no code with oracle/.
+// its own because its CTA shape differs from the FFMA2 kernel's: 4 warps at 80 registers, 6 CTAs = 24 warps per SM (the
+// finalisation is out of line, so the hot loop fits without spills). With one unit per row-group (pilot_device.cuh) the
+// gather runs at the rate at which the L1 takes missed 128-byte lines (about 1.85 clocks per line per SM, the ceiling of
+// pilot_refine_probe_unit_gather), and warps hide that better than registers of prefetched taps. Measured on config 4
+// (B200, ms per step): 16 warps at 128 registers 8.76 (8.31 with the next round's taps prefetched), 20 warps at 96: 8.17,
+// 24 at 80: 7.88, 28 at 72: 7.94, 32 at 64: 8.30; CTAs of 2 / 8 warps at the same occupancy 7.94 / 8.02; anchors per CTA
+// 768 ... 3072: 7.83-7.87 (1536 kept). Round 1's layout (a unit split over two row-groups, 28 warps at 72 registers): 7.65
+// with the empty batches skipped, 8.98 without. Shares no code with oracle/.
 #ifndef PILOT_MMA_THREADS
 #define PILOT_MMA_THREADS 128
 #define PILOT_MMA_MIN_BLOCKS 6
 #endif
 #ifndef PILOT_MMA_PIPE
 #define PILOT_MMA_PIPE 0
+#endif
+#ifndef PILOT_MMA_SB
+#define PILOT_MMA_SB 96             // anchors per super-batch of a warp: measured (B200, config 4 | config 2, ms) 32: 8.00 | 7.76,
+                                    // 64: 7.77 | 7.50, 96: 7.75 | 7.41, 128: 8.50 | 7.62
 #endif
 #define PILOT_THREADS PILOT_MMA_THREADS
 #define PILOT_MIN_BLOCKS PILOT_MMA_MIN_BLOCKS
