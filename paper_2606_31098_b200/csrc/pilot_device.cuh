@@ -1184,6 +1184,11 @@ __device__ __forceinline__ bool range_enabled(const PassArgs& A) {
   return A.prm.range_mode != PILOT_RANGE_OFF && A.prm.w_range > 0.f && A.dsm != nullptr;
 }
 
+// Lane 0 does everything after the warp-wide ray-march. A lane-parallel variant (component i of the system in lane i, the
+// record stores and state copies spread over the lanes, a right-looking 6x6 Cholesky by rows with shuffle broadcasts) was
+// written in round 2, parity green, and removed: in-kernel counters gave 8.3 k cycles per iteration against 6.7 k for this
+// one (priors 2.5 k vs 1.5 k, solve 3.3 k vs 3.3 k, record 1.1 k vs 0.85 k) - the chain of dependent fp64 operations
+// (~16 cycles each) is what costs, and shuffles and selects only lengthen it.
 // Warp-collective. `s` is the hypothesis' optimiser state (global or shared memory); `pre` = the range prior at
 // the candidate pose if it was computed already, else nullptr (computed here).
 __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const float* sums /* smem, kNacc */, int lane,
@@ -1316,21 +1321,18 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
 #undef PILOT_TP
 }
 
-// The same on the state in the workspace (global memory): lane 0 works on a private copy, so that the optimiser
-// state sits in registers / L1 instead of being re-read from L2 around every output store. Warp-collective.
-__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane) {
-  HypState loc;
-  const HypState& g = A.state[m];
-  if (lane == 0) {
-    loc = g;
-  } else {                       // the other lanes only need the candidate pose (ray-march of the range prior)
-#pragma unroll
-    for (int i = 0; i < 9; ++i) loc.Rc[i] = g.Rc[i];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) loc.Cc[i] = g.Cc[i];
-  }
-  finalize_hypothesis(A, loc, m, sums, lane, nullptr);
-  if (lane == 0) A.state[m] = loc;
+// The same on the state in the workspace (global memory): the warp stages it through `scratch` (SHARED memory, one
+// HypState per calling warp) with coalesced copies, so that lane 0 works on shared memory instead of chasing 456 bytes
+// of global memory through dependent loads (config 4 7.75 -> 7.57 ms, config 2 7.41 -> 7.33). Warp-collective.
+__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane, HypState* scratch) {
+  const int* src = reinterpret_cast<const int*>(A.state + m);
+  int* dst = reinterpret_cast<int*>(scratch);
+  for (int i = lane; i < (int)(sizeof(HypState) / 4); i += 32) dst[i] = src[i];
+  __syncwarp();
+  finalize_hypothesis(A, *scratch, m, sums, lane, nullptr);
+  __syncwarp();
+  int* out = reinterpret_cast<int*>(A.state + m);
+  for (int i = lane; i < (int)(sizeof(HypState) / 4); i += 32) out[i] = dst[i];
 }
 
 }  // namespace

@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   __shared__ float s_part[kWarps][kNacc];
   __shared__ float s_sum[kNacc];
   __shared__ int s_last;
+  __shared__ HypState s_state;                   // the last CTA's warp 0 finalises on a copy in shared memory
   s_part[warp][lane] = wtot;
   __syncthreads();
   if (warp == 0) {
@@ -55,7 +56,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   s_sum[lane] = t;
   if (lane == 0) A.counters[m] = 0u;
   __syncwarp();
-  finalize_in_workspace(A, m, s_sum, lane);
+  finalize_in_workspace(A, m, s_sum, lane, &s_state);
 }
 
 }  // namespace
