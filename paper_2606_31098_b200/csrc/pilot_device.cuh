@@ -405,6 +405,10 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
                                    // 7.88 without it at 24 warps (80 registers, where it spills): pilot_pass_mma.cu turns it off
 #endif
 
+#ifndef PILOT_MMA_PROJ_ILP
+#define PILOT_MMA_PROJ_ILP 0       // 1: the projection passes of a super-batch side by side (pass kernel: config 4 -0.8 %;
+                                    // the resident kernel, whose levels can be smaller than a super-batch, loses 1-3 %)
+#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
                                     // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
@@ -529,10 +533,61 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   const int n_batches = (end - begin + 31) >> 5;
   auto load_anchor = [&](int b) { const int j = begin + b * 32 + lane; return (b < n_batches && j < end) ? __ldg(L.points + j) : make_float4(0.f, 0.f, 0.f, -1.f); };
   constexpr int PASSES = SB / 32;
+  float4 Pn = load_anchor(worker);
   for (int b0 = worker; b0 < n_batches; b0 += PASSES * n_workers) {
     // ---- project + compact
     int nv = 0;
-    float4 Pn = load_anchor(b0);
+#if PILOT_MMA_PROJ_ILP
+    // the SB / 32 passes are independent fp64 chains: written out side by side so that the compiler interleaves them (a
+    // batch past the end projects nothing: its lanes are invalid). The first pass's anchors were loaded one super-batch ago.
+    {
+      float4 Pk[PASSES];
+      Pk[0] = Pn;
+#pragma unroll
+      for (int k = 1; k < PASSES; ++k) Pk[k] = load_anchor(b0 + k * n_workers);
+      Pn = load_anchor(b0 + PASSES * n_workers);
+      double R[12];                                                       // six 16-byte shared-memory loads
+#pragma unroll
+      for (int i = 0; i < 6; ++i)
+        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
+      const double* Cc = R + 9;
+      float pa[PASSES], pb[PASSES], px[PASSES], py[PASSES], piz[PASSES];
+      unsigned poff[PASSES];
+      bool pvalid[PASSES];
+#pragma unroll
+      for (int k = 0; k < PASSES; ++k) {
+        const int base = begin + (b0 + k * n_workers) * 32;
+        bool valid = (b0 + k * n_workers) < n_batches && base + lane < end;
+        double dx = (double)Pk[k].x - Cc[0], dy = (double)Pk[k].y - Cc[1], dz = (double)Pk[k].z - Cc[2];
+        double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
+        double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
+        double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
+        valid = valid && (Zd > (double)A.prm.z_near);
+        double izd = fast_rcp(Zd);
+        double ud = (double)L.fx * Xd * izd + (double)L.cx;
+        double vd = (double)L.fy * Yd * izd + (double)L.cy;
+        double x0d = floor(ud), y0d = floor(vd);
+        valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
+        const float iz = (float)izd;
+        pa[k] = (float)(ud - x0d); pb[k] = (float)(vd - y0d);
+        px[k] = (float)Xd * iz; py[k] = (float)Yd * iz; piz[k] = iz;
+        poff[k] = valid ? ((unsigned)(int)y0d * (unsigned)L.W + (unsigned)(int)x0d) * (unsigned)PX : 0u;
+        pvalid[k] = valid;
+      }
+#pragma unroll
+      for (int k = 0; k < PASSES; ++k) {
+        const unsigned vmask = __ballot_sync(0xffffffffu, pvalid[k]);
+        if (pvalid[k]) {
+          const int s = nv + __popc(vmask & ((1u << lane) - 1u));
+          slotA[s] = make_uint2(poff[k], (unsigned)(begin + (b0 + k * n_workers) * 32 + lane));
+          slotB[s] = make_float4(pa[k], pb[k], px[k], py[k]);
+          slotC[s] = make_float2(piz[k], Pk[k].w);
+        }
+        nv += __popc(vmask);
+      }
+    }
+#else
+    Pn = load_anchor(b0);
 #pragma unroll 1
     for (int k = 0; k < PASSES; ++k) {
       const int b = b0 + k * n_workers;
@@ -567,6 +622,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       }
       nv += __popc(vmask);
     }
+#endif
     if (nv == 0) continue;                                                // no visible unit: nothing to gather
     __syncwarp();
 

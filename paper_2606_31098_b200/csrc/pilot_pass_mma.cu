@@ -14,6 +14,9 @@
 #ifndef PILOT_MMA_PIPE
 #define PILOT_MMA_PIPE 0
 #endif
+#ifndef PILOT_MMA_PROJ_ILP
+#define PILOT_MMA_PROJ_ILP 1
+#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 96             // anchors per super-batch of a warp: measured (B200, config 4 | config 2, ms) 32: 8.00 | 7.76,
                                     // 64: 7.77 | 7.50, 96: 7.75 | 7.41, 128: 8.50 | 7.62
