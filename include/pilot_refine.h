@@ -438,8 +438,8 @@ int pilot_refine_reprojection_loss(const float* poses_dev, int n_poses, const fl
  * dL = <dL/dH, dH> for symmetric dH; q_prev_dev[m][6] (optional) = the part of dL / d eps at the PREVIOUS pose that flows
  * through the retraction, Ad(exp(dxi^))^T q; status_dev[m] (optional) = PILOT_STATUS_CHOL_FAIL if H + lambda D is not
  * positive definite. hessian_dev [n][36] row-major (symmetrised on read), gradient_dev [n][6], lambda_dev [n]: what
- * pilot_refine_run records per iteration. Not built: the dependence of H and g on the pose and on the feature maps (the
- * transpose of the gather). Asynchronous on cuda_stream; double arithmetic, one rounding to fp32 on output.
+ * pilot_refine_run records per iteration. The dependence of H and g on the pose and on the feature maps is
+ * pilot_refine_photo_backward below. Asynchronous on cuda_stream; double arithmetic, one rounding to fp32 on output.
  */
 int pilot_refine_reprojection_loss_grad(const float* poses_dev, int n_poses, const float pose_star[12],
                                         const float* points_dev, int n_points, const float intrinsics[4],
@@ -448,6 +448,29 @@ int pilot_refine_reprojection_loss_grad(const float* poses_dev, int n_poses, con
 int pilot_refine_lm_step_adjoint(const float* hessian_dev, const float* gradient_dev, const float* lambda_dev,
                                  const float* q_dev, int n, int damp_mode, float* dxi_dev, float* grad_hessian_dev,
                                  float* grad_gradient_dev, float* q_prev_dev, unsigned* status_dev, void* cuda_stream);
+
+/*
+ * Backward pass of the photo term: the transpose of the gather (Eq.1, Eq.2, Eq.8, PAPER.md:118-122,
+ * 160-164). For every pose m < n_poses (poses_dev [n][12] = [R_wc | C], the poses at which the systems were built) and one
+ * pyramid level, with S_m = <grad_hessian_dev[m], H_m> + <grad_gradient_dev[m], g_m> (H_m, g_m the PHOTO part of the normal
+ * equations at that pose, GRAD_BILINEAR_EXACT; grad_hessian_dev [n][36] is symmetrised on read), it ADDS to
+ *   grad_feat_dev [height][width][channels] fp32   sum_m dS_m / dF        (the query feature map)
+ *   grad_ref_dev  [n_points][channels]      fp32   sum_m dS_m / df^r
+ *   grad_conf_dev [height][width]           fp32   sum_m dS_m / dconf     (only with query_conf_dev; may be NULL)
+ * (the caller zeroes or pre-loads them; any may be NULL) and WRITES grad_pose_dev[m][6] = dS_m / d eps for the left
+ * perturbation T_cw <- exp(eps^) T_cw, eps = (rho; phi) (may be NULL). The bilinear cell and the visible set are held fixed
+ * (piecewise constant); the robust weight's second derivative and the dependence of the projection Jacobian on the point
+ * are included. The priors are not part of S (they do not depend on the features). Sums use fp32 atomics: the result is
+ * reproducible to rounding, not bit for bit. Together with pilot_refine_reprojection_loss_grad and
+ * pilot_refine_lm_step_adjoint this is the chain rule through one unrolled LM step for a photo-only objective.
+ * points_dev 16-byte aligned; map under 4 GiB of elements. Asynchronous on cuda_stream.
+ */
+int pilot_refine_photo_backward(const void* query_feat_dev, const float* query_conf_dev, int width, int height, int channels,
+                                pilot_dtype feat_dtype, const float intrinsics[4], const float* points_dev,
+                                const void* ref_feat_dev, int n_points, const float* poses_dev,
+                                const float* grad_hessian_dev, const float* grad_gradient_dev, int n_poses,
+                                pilot_loss loss, float loss_scale, float z_near, float* grad_feat_dev, float* grad_ref_dev,
+                                float* grad_conf_dev, float* grad_pose_dev, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Anchor order (kernel description PAPER.md:485). The sums of Eq.(2) and Eq.(8) do not depend on the

@@ -36,7 +36,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
            "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
            "pilot_refine_set_grid_host", "pilot_refine_submit_pruned_host",
-           "pilot_refine_reprojection_loss_grad", "pilot_refine_lm_step_adjoint",
+           "pilot_refine_reprojection_loss_grad", "pilot_refine_lm_step_adjoint", "pilot_refine_photo_backward",
            "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
 SEQ_ROW = 16
 
@@ -187,6 +187,11 @@ def lib():
         L.pilot_refine_lm_step_adjoint.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p,
                                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.pilot_refine_lm_step_adjoint.restype = C.c_int
+        L.pilot_refine_photo_backward.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float),
+                                                  C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                                  C.c_int, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                  C.c_void_p]
+        L.pilot_refine_photo_backward.restype = C.c_int
         L.pilot_refine_set_grid_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.pilot_refine_set_grid_host.restype = C.c_int
         L.pilot_refine_submit_pruned_host.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.c_void_p, C.c_int,
@@ -863,4 +868,27 @@ def lm_step_adjoint(hessian, gradient, lam, q, damp="identity", stream=None):
                                               o["dxi"].data_ptr(), o["grad_hessian"].data_ptr(), o["grad_gradient"].data_ptr(),
                                               o["q_prev"].data_ptr(), o["status"].data_ptr(), _stream_ptr(torch, stream, dev)),
            "pilot_refine_lm_step_adjoint")
+    return o
+
+
+def photo_backward(di, level, poses, grad_hessian, grad_gradient, loss="huber", loss_scale=0.1, z_near=0.1, stream=None,
+                   want_conf=True):
+    """Backward of the photo term of level `level` of DeviceInputs `di` (pilot_refine_photo_backward). poses [n, 12],
+    grad_hessian [n, 36], grad_gradient [n, 6]: cuda float32. -> dict(grad_feat [H, W, C], grad_ref [N, C], grad_conf
+    [H, W] or None, grad_pose [n, 6]) fresh, zero-initialised fp32 tensors."""
+    torch = _torch()
+    dev = poses.device
+    Hh, W, Cn, N = di.height[level], di.width[level], di.channels[level], int(di.inp.n_points[level])
+    has_conf = bool(di.inp.query_conf_dev[level]) and want_conf
+    o = dict(grad_feat=torch.zeros(Hh, W, Cn, dtype=torch.float32, device=dev), grad_ref=torch.zeros(N, Cn, dtype=torch.float32, device=dev),
+             grad_conf=torch.zeros(Hh, W, dtype=torch.float32, device=dev) if has_conf else None,
+             grad_pose=torch.empty(int(poses.shape[0]), 6, dtype=torch.float32, device=dev))
+    K = (C.c_float * 4)(*[float(di.inp.intrinsics[level][k]) for k in range(4)])
+    _check(lib().pilot_refine_photo_backward(di.inp.query_feat_dev[level], di.inp.query_conf_dev[level], W, Hh, Cn, DTYPE_CODE[di.dtype],
+                                             K, di.inp.points_dev[level], di.inp.ref_feat_dev[level], N, poses.contiguous().data_ptr(),
+                                             grad_hessian.contiguous().data_ptr(), grad_gradient.contiguous().data_ptr(),
+                                             int(poses.shape[0]), LOSS_CODE[loss], float(loss_scale), float(z_near),
+                                             o["grad_feat"].data_ptr(), o["grad_ref"].data_ptr(),
+                                             o["grad_conf"].data_ptr() if has_conf else None, o["grad_pose"].data_ptr(),
+                                             _stream_ptr(torch, stream, dev)), "pilot_refine_photo_backward")
     return o
