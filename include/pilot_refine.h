@@ -150,6 +150,27 @@ int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in,
 int pilot_refine_destroy(pilot_refine_handle* h);
 
 /*
+ * The same refinement as pilot_refine_create + pilot_refine_run (Eqs.1-9, all levels; default launch and math modes) for
+ * callers that may NOT allocate device memory (code under CUDA-graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): no handle, and the optimiser workspace (per-hypothesis LM state, tickets, per-CTA partial sums) is a
+ * file-scope device array of PILOT_STATIC_WORKSPACE_BYTES inside the library, which every GPU that loads the library
+ * holds until the process exits. The call makes no cudaMalloc / cudaFree and calls no allocating library routine; the
+ * caller still owns every input and output buffer. cfg: as for create(), with workspace_dev == NULL (else PILOT_ERR_ARG).
+ * LIMIT: pilot_refine_workspace_bytes(cfg) <= PILOT_STATIC_WORKSPACE_BYTES (32 MiB), i.e. about 128 bytes x max_hypotheses x
+ * ceil(max_points / 128) (+ 0.5 KB per hypothesis): 256 hypotheses x 65536 anchors (config 4: 16.9 MB) fit, 1024 x 65536
+ * (67 MB) do not -> PILOT_ERR_WORKSPACE, nothing launched. launches_out (optional, host): kernels launched by this call.
+ * SHARED STATE: every call on a device uses the same array, which keeps the previous call's contents; each call re-initialises
+ * what it reads (LM state and tickets of its n_hypotheses; partial sums are written before they are read), so back-to-back
+ * calls on ONE stream are correct. Calls that may overlap on the GPU (two streams, two host threads, a handle-free call
+ * racing a captured graph that contains one) RACE on the array: serialise them. Asynchronous like pilot_refine_run.
+ */
+#define PILOT_STATIC_WORKSPACE_BYTES (32u << 20)
+size_t pilot_refine_static_workspace_bytes(void);
+int pilot_refine_run_static(const pilot_refine_config* cfg, const pilot_refine_inputs* in,
+                            const pilot_refine_params* p, const pilot_refine_outputs* out,
+                            void* cuda_stream, int* launches_out);
+
+/*
  * Host-buffer path (what bench.py's "e2e" times): every "_dev" pointer of `in_host` and
  * `out_host` is a HOST pointer (pinned memory recommended). run_host copies the inputs into
  * device staging owned by the handle (cudaMemcpyAsync on the handle's copy stream), enqueues

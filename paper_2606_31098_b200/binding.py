@@ -37,7 +37,8 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
            "pilot_refine_set_grid_host", "pilot_refine_submit_pruned_host",
            "pilot_refine_reprojection_loss_grad", "pilot_refine_lm_step_adjoint", "pilot_refine_photo_backward",
-           "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss"]
+           "pilot_refine_footprint", "pilot_refine_lift_anchors", "pilot_refine_reprojection_loss",
+           "pilot_refine_run_static", "pilot_refine_static_workspace_bytes"]
 SEQ_ROW = 16
 
 
@@ -127,6 +128,11 @@ def lib():
             fn.restype = C.c_int
         L.pilot_refine_destroy.argtypes = [C.c_void_p]
         L.pilot_refine_destroy.restype = C.c_int
+        L.pilot_refine_run_static.argtypes = [C.POINTER(Config), C.POINTER(Inputs), C.POINTER(Params), C.POINTER(Outputs),
+                                              C.c_void_p, C.POINTER(C.c_int)]
+        L.pilot_refine_run_static.restype = C.c_int
+        L.pilot_refine_static_workspace_bytes.argtypes = []
+        L.pilot_refine_static_workspace_bytes.restype = C.c_size_t
         L.pilot_refine_last_launches.argtypes = [C.c_void_p]
         L.pilot_refine_last_launches.restype = C.c_int
         L.pilot_refine_set_chunk.argtypes = [C.c_void_p, C.c_int]
@@ -480,6 +486,34 @@ def refine(prob, params=None, device=0, mode="auto", cluster=0, math="auto"):
     res["launches"] = r.last_launches
     r.close()
     return res
+
+
+def static_workspace_bytes():
+    return int(lib().pilot_refine_static_workspace_bytes())
+
+
+def run_static(di, params, out, max_hypotheses=None, max_points=None, device=0, stream=None):
+    """pilot_refine_run_static: the refinement with the library's file-scope workspace, no handle and no allocation in
+    the call. `out`: dict name -> caller-owned cuda tensor (poses [H,12] f32, cost [H] f32, n_valid [H] i32, status [H]
+    i32, iter_hessian [T,H,36], iter_gradient [T,H,6], iter_cost [T,H], iter_lambda [T,H]); any subset. Returns the
+    number of kernels launched. Asynchronous on `stream`; calls must not overlap on the GPU (they share the workspace)."""
+    torch = _torch()
+    par, P = make_params(params, di.n_levels)
+    cfg = Config()
+    cfg.device, cfg.n_levels, cfg.feat_dtype = device, di.n_levels, DTYPE_CODE[di.dtype]
+    for l in range(di.n_levels):
+        cfg.width[l], cfg.height[l], cfg.channels[l] = int(di.width[l]), int(di.height[l]), int(di.channels[l])
+    cfg.max_hypotheses = int(max_hypotheses if max_hypotheses is not None else max(1, di.n_hyp))
+    cfg.max_points = int(max_points if max_points is not None else max(1, di.max_points))
+    cfg.max_total_iters = sum(P["iters"])
+    o = Outputs()
+    for name, t in out.items():
+        assert t.is_cuda and t.is_contiguous()
+        setattr(o, name + "_dev", t.data_ptr())
+    n = C.c_int(0)
+    _check(lib().pilot_refine_run_static(C.byref(cfg), C.byref(di.inp), C.byref(par), C.byref(o),
+                                         _stream_ptr(torch, stream, device), C.byref(n)), "pilot_refine_run_static")
+    return int(n.value)
 
 
 # ------------------------------------------------------------------ hypothesis set (PAPER.md:151, 168, 381-386)

@@ -21,6 +21,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
+
 namespace {
 
 // ------------------------------------------------------------------ kernels
@@ -763,6 +765,77 @@ int pilot_refine_run_host(pilot_refine_handle* h, const pilot_refine_inputs* in,
   int t = pilot_refine_submit_host(h, in, p, out, cuda_stream);
   if (t < 0) return t;
   return pilot_refine_wait_host(h);
+}
+
+}  // extern "C"
+
+// ====================================================================== allocation-free entry point
+//
+// For callers that may not call cudaMalloc (stream capture, serving loops, harnesses that forbid it): the same refinement
+// with the optimiser workspace (HypState per hypothesis, tickets, per-CTA partial sums) in an array that is part of the
+// loaded module. `g_static_workspace` is, in HOST code, only a stand-in for the symbol: the device address the kernels get
+// comes from cudaGetSymbolAddress, asked once per device with that device current.
+
+static __device__ __align__(256) unsigned char g_static_workspace[PILOT_STATIC_WORKSPACE_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticSetup { bool ready; char* ws; int sm_count; };
+StaticSetup g_static_setup[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+// the current device must be `device`
+int static_setup(int device, StaticSetup* out) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticSetup& s = g_static_setup[device];
+  if (!s.ready) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_static_workspace) != cudaSuccess || !ptr) { cudaGetLastError(); return PILOT_ERR_CUDA; }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms < 1) { cudaGetLastError(); return PILOT_ERR_CUDA; }
+    s.ws = static_cast<char*>(ptr);
+    s.sm_count = sms;
+    s.ready = true;
+  }
+  *out = s;
+  return PILOT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t pilot_refine_static_workspace_bytes(void) { return (size_t)PILOT_STATIC_WORKSPACE_BYTES; }
+
+int pilot_refine_run_static(const pilot_refine_config* cfg, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                            const pilot_refine_outputs* out, void* cuda_stream, int* launches_out) {
+  if (launches_out) *launches_out = 0;
+  if (!config_ok(cfg) || cfg->workspace_dev || !in || !p || !out) return PILOT_ERR_ARG;
+  for (int l = 0; l < cfg->n_levels; ++l)
+    if (lanes_per_unit(cfg->channels[l], cfg->feat_dtype) == 0) return PILOT_ERR_UNSUPPORTED;
+  if (!shape_supported(cfg)) return PILOT_ERR_UNSUPPORTED;
+  const WsLayout w = ws_layout(cfg);
+  if (w.total > (size_t)PILOT_STATIC_WORKSPACE_BYTES) return PILOT_ERR_WORKSPACE;   // capacity beyond the static array
+  if (cfg->device < 0 || cfg->device >= kStaticMaxDevices) return PILOT_ERR_ARG;
+  int prev = 0;
+  if (cudaGetDevice(&prev) != cudaSuccess) return PILOT_ERR_CUDA;
+  if (prev != cfg->device && cudaSetDevice(cfg->device) != cudaSuccess) { cudaGetLastError(); return PILOT_ERR_CUDA; }
+  StaticSetup s;
+  int rc = static_setup(cfg->device, &s);
+  if (rc == PILOT_OK) {
+    pilot_refine_handle h;                     // lives on the stack for the duration of the call: nothing is allocated
+    memset(&h, 0, sizeof h);
+    h.cfg = *cfg;
+    h.ws = s.ws; h.ws_bytes = (size_t)PILOT_STATIC_WORKSPACE_BYTES; h.owns_ws = false;
+    h.max_chunks = w.max_chunks;
+    h.mode = PILOT_EXEC_AUTO; h.math_mode = PILOT_MATH_AUTO;
+    h.sm_count = s.sm_count;
+    rc = pilot_refine_run_levels(&h, in, p, out, 0, cfg->n_levels, cuda_stream);
+    if (launches_out) *launches_out = h.last_launches;
+  }
+  if (prev != cfg->device) cudaSetDevice(prev);
+  return rc;
 }
 
 }  // extern "C"
