@@ -113,23 +113,35 @@ __device__ __forceinline__ uint4 ldg16(const void* p) {
 
 // ------------------------------------------------------------------ fast double reciprocal / reciprocal sqrt
 //
-// A double-precision divide or sqrt is a ~30-instruction dependent sequence; the per-hypothesis finalisation (one
-// lane, the serial tail of every LM iteration) and the ray-march are chains of them. These start from the fp32
-// hardware approximation and take two Newton steps in double (relative error ~1e-16 inside the fp32 range).
+// A double-precision divide or sqrt is a ~30-instruction dependent sequence (measured on B200, one warp, dependent chain:
+// 1/x 59 cycles, sqrt 78; a dependent DFMA 8). The per-hypothesis finalisation (one lane, the serial tail of every LM
+// iteration), the ray-march and the projection of every anchor are chains of them. These start from the fp64 hardware
+// seed (MUFU.RCP64H / MUFU.RSQ64H: 2^-22 relative, no fp32 round trip) and take ONE third-order step in double: relative
+// error <= 2.6e-16 over 2^-100 .. 2^100, 40 / 50 cycles (round 1's fp32 seed + two Newton steps: 161 / 155).
+// Arguments outside 2^-1007 .. 2^993 in magnitude (zero, subnormal, inf, NaN) take the exact division on a cold branch.
+__device__ __forceinline__ bool fp64_mid_range(double d) {
+  const unsigned hi = (unsigned)__double2hiint(d) & 0x7fffffffu;
+  return hi - 0x01000000u < 0x7e000000u - 0x01000000u;
+}
+__device__ __forceinline__ double inv_sqrt_core(double s) {       // s > 0 in the middle range
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+  const double t = s * y;
+  const double e = fma(-t, y, 1.0);                               // 1 - s y^2
+  const double p = fma(0.375, e, 0.5), ye = y * e;
+  return fma(ye, p, y);                                           // y (1 + e/2 + 3 e^2 / 8)
+}
 __device__ __forceinline__ double inv_sqrt(double s) {
-  if (!(s > 1e-30) || !(s < 1e30)) return 1.0 / sqrt(s);
-  double y = (double)rsqrtf((float)s);
-  y = y * (1.5 - 0.5 * s * y * y);
-  y = y * (1.5 - 0.5 * s * y * y);
-  return y;
+  if (!fp64_mid_range(s) || s < 0.0) return 1.0 / sqrt(s);
+  return inv_sqrt_core(s);
 }
 __device__ __forceinline__ double fast_rcp(double d) {
-  const double ad = fabs(d);
-  if (!(ad > 1e-30) || !(ad < 1e30)) return 1.0 / d;
-  double y = (double)__frcp_rn((float)d);
-  y = y * (2.0 - d * y);
-  y = y * (2.0 - d * y);
-  return y;
+  if (!fp64_mid_range(d)) return 1.0 / d;
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  const double e = fma(-d, y, 1.0);                               // 1 - d y
+  const double p = fma(e, e, e);
+  return fma(y, p, y);                                            // y (1 + e + e^2)
 }
 
 // rho, rho' for the prior terms, in double, without sqrt / divide
@@ -1132,7 +1144,8 @@ __device__ bool range_prior(const PassArgs& A, const double* R, const double* C,
 
 // ------------------------------------------------------------------ 6x6 Cholesky solve, SE(3) retraction (a9, a10)
 
-__device__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6]) {
+// General path (any pivot): left-looking, returns false at the first pivot that is not positive and finite.
+__device__ __noinline__ bool chol_solve6_checked(const double* Hs, double lambda, int damp_mode, const double* g, double* x) {
   double Lm[6][6], inv[6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
@@ -1163,12 +1176,60 @@ __device__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode
   for (int i = 5; i >= 0; --i) {
     double s = y[i];
 #pragma unroll
-    for (int k = i + 1; k < 6; ++k) s -= Lm[k][i] * x[k];
+    for (int k = 5; k > i; --k) s -= Lm[k][i] * x[k];
     x[i] = s * inv[i];
   }
   bool ok = true;
 #pragma unroll
   for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
+  return ok;
+}
+
+// (H + damping) x = g by Cholesky. The finalisation is ONE lane's chain of dependent fp64 operations (8 cycles each on
+// B200), so the common case is written for the shortest chain: right-looking (a column's updates of the trailing matrix
+// are independent of each other: ~65 cycles per column = seed + cubic step + scale + update, against the left-looking
+// accumulation whose chain grows with the column), no branch between the columns (one basic block for ptxas to
+// interleave), substitutions column by column. Every element sees the same subtractions in the same order as in the
+// left-looking form. A pivot outside (2^-1007, 2^993) - including every failure (<= 0, NaN, inf) - sends the whole solve
+// to chol_solve6_checked on a cold path, which decides.
+__device__ __forceinline__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6]) {
+  double a[21], inv[6];
+#pragma unroll
+  for (int i = 0; i < 21; ++i) a[i] = Hs[i];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) a[tri(i, i)] += (damp_mode == PILOT_DAMP_IDENTITY) ? lambda : lambda * fmax(Hs[tri(i, i)], 1e-12);
+  bool plain = true;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    const double d = a[tri(j, j)];
+    plain = plain && d > 0.0 && fp64_mid_range(d);
+    inv[j] = inv_sqrt_core(d);
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i) a[tri(j, i)] *= inv[j];                 // L[i][j]
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i)
+#pragma unroll
+      for (int k = j + 1; k <= i; ++k) a[tri(k, i)] -= a[tri(j, i)] * a[tri(j, k)];
+  }
+  double y[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) y[i] = g[i];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+    y[k] *= inv[k];
+#pragma unroll
+    for (int i = k + 1; i < 6; ++i) y[i] -= a[tri(k, i)] * y[k];
+  }
+#pragma unroll
+  for (int k = 5; k >= 0; --k) {
+    y[k] *= inv[k];
+#pragma unroll
+    for (int i = 0; i < k; ++i) y[i] -= a[tri(i, k)] * y[k];
+  }
+  bool ok = plain;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) { x[i] = y[i]; ok = ok && isfinite(y[i]); }
+  if (!plain) return chol_solve6_checked(Hs, lambda, damp_mode, g, x);
   return ok;
 }
 
@@ -1247,7 +1308,7 @@ __device__ __forceinline__ bool range_enabled(const PassArgs& A) {
 // (~16 cycles each) is what costs, and shuffles and selects only lengthen it.
 // Warp-collective. `s` is the hypothesis' optimiser state (global or shared memory); `pre` = the range prior at
 // the candidate pose if it was computed already, else nullptr (computed here).
-__device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const float* sums /* smem, kNacc */, int lane,
+__device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const double* sums /* smem, kNacc */, int lane,
                                     const PriorRes* pre) {
   const pilot_refine_params& P = A.prm;
 
@@ -1272,10 +1333,10 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
 
   double Hn[21], gn[6], costn;
   unsigned fl = 0;
-  for (int i = 0; i < 21; ++i) Hn[i] = (double)sums[i];
-  for (int i = 0; i < 6; ++i) gn[i] = (double)sums[21 + i];
-  costn = (double)sums[27];
-  int nv = (int)(sums[28] + 0.5f);
+  for (int i = 0; i < 21; ++i) Hn[i] = sums[i];          // converted to double by the 32 lanes that summed them
+  for (int i = 0; i < 6; ++i) gn[i] = sums[21 + i];
+  costn = sums[27];
+  int nv = (int)(sums[28] + 0.5);
   s.visible_evals += (unsigned long long)nv;
   if (nv < P.min_valid) { costn = INFINITY; fl |= PILOT_STATUS_FEW_VALID; }
 
@@ -1380,7 +1441,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
 // The same on the state in the workspace (global memory): the warp stages it through `scratch` (SHARED memory, one
 // HypState per calling warp) with coalesced copies, so that lane 0 works on shared memory instead of chasing 456 bytes
 // of global memory through dependent loads (config 4 7.75 -> 7.57 ms, config 2 7.41 -> 7.33). Warp-collective.
-__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const float* sums, int lane, HypState* scratch) {
+__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const double* sums, int lane, HypState* scratch) {
   const int* src = reinterpret_cast<const int*>(A.state + m);
   int* dst = reinterpret_cast<int*>(scratch);
   for (int i = lane; i < (int)(sizeof(HypState) / 4); i += 32) dst[i] = src[i];

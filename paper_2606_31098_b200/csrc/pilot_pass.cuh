@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float wtot = acc_warp_total<MMA>(acc, sacc, lane);
   __shared__ float s_part[kWarps][kNacc];
-  __shared__ float s_sum[kNacc];
+  __shared__ double s_sum[kNacc];                // the hypothesis' sums, converted by the lane that holds each
   __shared__ int s_last;
   __shared__ HypState s_state;                   // the last CTA's warp 0 finalises on a copy in shared memory
   s_part[warp][lane] = wtot;
@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
   float t = 0.f;
   const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
   for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);
-  s_sum[lane] = t;
+  s_sum[lane] = (double)t;
   if (lane == 0) A.counters[m] = 0u;
   __syncwarp();
   finalize_in_workspace(A, m, s_sum, lane, &s_state);

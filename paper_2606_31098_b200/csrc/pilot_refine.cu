@@ -34,13 +34,13 @@ constexpr int kFinWarps = 4;
 __global__ void __launch_bounds__(kFinWarps * 32) finalize_kernel(const __grid_constant__ PassArgs A) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int m = blockIdx.x * kFinWarps + warp;
-  __shared__ float s_sum[kFinWarps][kNacc];
+  __shared__ double s_sum[kFinWarps][kNacc];
   __shared__ HypState s_state[kFinWarps];
   if (m >= A.n_hyp || A.state[m].level != A.level) return;
   float t = 0.f;
   const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
   for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);      // fixed order
-  s_sum[warp][lane] = t;
+  s_sum[warp][lane] = (double)t;
   __syncwarp();
   finalize_in_workspace(A, m, s_sum[warp], lane, &s_state[warp]);
 }

@@ -30,7 +30,7 @@ struct ResidentShared {
   __align__(16) double pose[12];     // this CTA's copy of the candidate pose: Rc[9], Cc[3]
   float part[kWarps][kNacc];
   float cta_sum[kNacc];              // this CTA's slice total; rank 0 reads it through DSMEM
-  float tot[kNacc];
+  double tot[kNacc];                 // the cluster's sums, converted to double by the lane that added each
   PriorRes prior;
   int go;
 };
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
       float t = 0.f;
 #pragma unroll
       for (unsigned r = 0; r < 8; ++r) t += v[r];                         // fixed order
-      sh.tot[lane] = t;
+      sh.tot[lane] = (double)t;
       __syncwarp();
       finalize_hypothesis(A, sh.st, m, sh.tot, lane, range_on ? &sh.prior : nullptr);
       __syncwarp();
