@@ -83,6 +83,9 @@ struct PassArgs {
   int n_hyp, level, level_end, pass, iters, rec_base;
   int chunk, n_chunks;
   int defer;                // 1: the pass kernel only writes partial sums; finalize_kernel ends the iteration
+  // what the finalisation reads as doubles, converted once on the host (an F2F costs the single finalising lane ~18 cycles)
+  struct { double lambda_init, lambda_up, lambda_down, lambda_min, lambda_max, w_gravity, gravity_scale, w_range, range_scale,
+                  gw[3], gi[3]; } pd;
   HypState* state;
   float* partials;          // [n_hyp][n_chunks][kNacc]
   unsigned* counters;       // [n_hyp]
@@ -1192,7 +1195,8 @@ __device__ __noinline__ bool chol_solve6_checked(const double* Hs, double lambda
 // interleave), substitutions column by column. Every element sees the same subtractions in the same order as in the
 // left-looking form. A pivot outside (2^-1007, 2^993) - including every failure (<= 0, NaN, inf) - sends the whole solve
 // to chol_solve6_checked on a cold path, which decides.
-__device__ __forceinline__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6]) {
+__device__ __forceinline__ bool chol_solve6(const double (&Hs)[21], double lambda, int damp_mode, const double (&g)[6], double (&x)[6],
+                                            const double* H_mem, const double* g_mem /* the same system in memory, for the cold path */) {
   double a[21], inv[6];
 #pragma unroll
   for (int i = 0; i < 21; ++i) a[i] = Hs[i];
@@ -1229,49 +1233,68 @@ __device__ __forceinline__ bool chol_solve6(const double (&Hs)[21], double lambd
   bool ok = plain;
 #pragma unroll
   for (int i = 0; i < 6; ++i) { x[i] = y[i]; ok = ok && isfinite(y[i]); }
-  if (!plain) return chol_solve6_checked(Hs, lambda, damp_mode, g, x);
+  if (!plain) {                        // cold: works from memory so that the arrays above stay in registers
+    double xs[6];
+    const bool r = chol_solve6_checked(H_mem, lambda, damp_mode, g_mem, xs);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) x[i] = xs[i];
+    return r;
+  }
   return ok;
 }
 
-// T_cw <- exp(xi) T_cw (Eq.9): R' = E R, C' = C - R^T E^T V rho
-__device__ void retract(const double* R, const double* C, const double (&xi)[6], double* Rn, double* Cn) {
+// sin(th)/th, (1 - cos th)/th^2, (th - sin th)/th^3 as even power series in th, TERMS terms each (three independent
+// Horner chains)
+template <int TERMS>
+__device__ __forceinline__ void so3_series(double th2, double& a, double& b, double& c) {
+  constexpr double f[22] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
+                            1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0,
+                            1.0 / 87178291200.0, 1.0 / 1307674368000.0, 1.0 / 20922789888000.0,
+                            1.0 / 355687428096000.0, 1.0 / 6402373705728000.0, 1.0 / 121645100408832000.0,
+                            1.0 / 2432902008176640000.0, 1.0 / 51090942171709440000.0};
+  a = f[2 * TERMS - 1]; b = f[2 * TERMS]; c = f[2 * TERMS + 1];
+#pragma unroll
+  for (int k = TERMS - 2; k >= 0; --k) {
+    a = f[2 * k + 1] - th2 * a;
+    b = f[2 * k + 2] - th2 * b;
+    c = f[2 * k + 3] - th2 * c;
+  }
+}
+
+// T_cw <- exp(xi) T_cw (Eq.9): R' = E R, C' = C - R^T E^T V rho with E = exp([phi]x) = I + a K + b K^2, V = I + b K + c K^2,
+// K^2 = phi phi^T - th^2 I, and E^T V = V(-phi) (E^T V(phi) = int_0^1 exp((t-1) K) dt), so that
+// E^T V rho = rho - b (phi x rho) + c (phi x (phi x rho)). Written for few instructions: one lane runs it as a dependent chain.
+__device__ __forceinline__ void retract(const double* R, const double* C, const double (&xi)[6], double* Rn, double* Cn) {
   const double px = xi[3], py = xi[4], pz = xi[5];
   const double th2 = px * px + py * py + pz * pz;
-  double a, b, c;      // sin(th)/th, (1 - cos th)/th^2, (th - sin th)/th^3: even power series in th
-  if (th2 <= 0.25) {
-    // LM steps are small rotations: 10 terms of the series (next term < 3e-23 at th = 0.5) instead of sqrt/sin/cos
-    constexpr double f[22] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
-                              1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0,
-                              1.0 / 87178291200.0, 1.0 / 1307674368000.0, 1.0 / 20922789888000.0,
-                              1.0 / 355687428096000.0, 1.0 / 6402373705728000.0, 1.0 / 121645100408832000.0,
-                              1.0 / 2432902008176640000.0, 1.0 / 51090942171709440000.0};
-    a = f[19]; b = f[20]; c = f[21];
-#pragma unroll
-    for (int k = 8; k >= 0; --k) {
-      a = f[2 * k + 1] - th2 * a;
-      b = f[2 * k + 2] - th2 * b;
-      c = f[2 * k + 3] - th2 * c;
-    }
+  double a, b, c;
+  if (th2 <= 1e-2) {
+    so3_series<5>(th2, a, b, c);         // LM steps are small rotations: next term < 3e-18 at th = 0.1
+  } else if (th2 <= 0.25) {
+    so3_series<10>(th2, a, b, c);        // next term < 3e-23 at th = 0.5
   } else {
     const double th = sqrt(th2);
     double sn, cs;
     sincos(th, &sn, &cs);
     a = sn / th; b = (1.0 - cs) / th2; c = (th - sn) / (th2 * th);
   }
-  double K[9] = {0, -pz, py, pz, 0, -px, -py, px, 0}, K2[9], E[9], V[9];
+  // E: diagonal 1 + b (p_i^2 - th2), off-diagonal b p_i p_j -+ a p_k
+  const double bxy = b * (px * py), bxz = b * (px * pz), byz = b * (py * pz);
+  const double E[9] = {fma(b, px * px - th2, 1.0), fma(-a, pz, bxy), fma(a, py, bxz),
+                       fma(a, pz, bxy), fma(b, py * py - th2, 1.0), fma(-a, px, byz),
+                       fma(-a, py, bxz), fma(a, px, byz), fma(b, pz * pz - th2, 1.0)};
+  // w = E^T V rho = rho - b k1 + c k2, k1 = phi x rho, k2 = phi x k1
+  const double k1x = py * xi[2] - pz * xi[1], k1y = pz * xi[0] - px * xi[2], k1z = px * xi[1] - py * xi[0];
+  const double k2x = py * k1z - pz * k1y, k2y = pz * k1x - px * k1z, k2z = px * k1y - py * k1x;
+  const double wx = fma(c, k2x, fma(-b, k1x, xi[0])), wy = fma(c, k2y, fma(-b, k1y, xi[1])), wz = fma(c, k2z, fma(-b, k1z, xi[2]));
+  double Rt[9];
+#pragma unroll
   for (int i = 0; i < 3; ++i)
-    for (int j = 0; j < 3; ++j) K2[3 * i + j] = K[3 * i] * K[j] + K[3 * i + 1] * K[3 + j] + K[3 * i + 2] * K[6 + j];
-  for (int i = 0; i < 9; ++i) {
-    double I = (i % 4 == 0) ? 1.0 : 0.0;
-    E[i] = I + a * K[i] + b * K2[i];
-    V[i] = I + b * K[i] + c * K2[i];
-  }
-  double Vr[3], EtVr[3], Rt[9];
-  for (int i = 0; i < 3; ++i) Vr[i] = V[3 * i] * xi[0] + V[3 * i + 1] * xi[1] + V[3 * i + 2] * xi[2];
-  for (int i = 0; i < 3; ++i) EtVr[i] = E[i] * Vr[0] + E[3 + i] * Vr[1] + E[6 + i] * Vr[2];
-  for (int i = 0; i < 3; ++i)
+#pragma unroll
     for (int j = 0; j < 3; ++j) Rt[3 * i + j] = E[3 * i] * R[j] + E[3 * i + 1] * R[3 + j] + E[3 * i + 2] * R[6 + j];
-  for (int i = 0; i < 3; ++i) Cn[i] = C[i] - (R[i] * EtVr[0] + R[3 + i] * EtVr[1] + R[6 + i] * EtVr[2]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) Cn[i] = C[i] - (R[i] * wx + R[3 + i] * wy + R[6 + i] * wz);
+#pragma unroll
   for (int i = 0; i < 9; ++i) Rn[i] = Rt[i];
 }
 
@@ -1294,89 +1317,122 @@ __device__ void write_final(const PassArgs& A, const HypState& s, int m) {
   if (A.out.status_dev) A.out.status_dev[m] = s.status | s.flags;
 }
 
-// Range prior evaluated ahead of the finalisation (the resident kernel overlaps it with the photo gather).
-struct PriorRes { int ok; double r; double J[6]; };
+// What the two priors add to the photo sums at a candidate pose (supp Eq.5-6): they depend on the pose only, so the resident
+// kernel evaluates them on a warp of their own WHILE the others gather, and the finalisation just adds 28 numbers.
+struct PriorTerms { double H[21]; double g[6]; double cost; unsigned flags; };
 
 __device__ __forceinline__ bool range_enabled(const PassArgs& A) {
   return A.prm.range_mode != PILOT_RANGE_OFF && A.prm.w_range > 0.f && A.dsm != nullptr;
 }
 
-// Lane 0 does everything after the warp-wide ray-march. A lane-parallel variant (component i of the system in lane i, the
-// record stores and state copies spread over the lanes, a right-looking 6x6 Cholesky by rows with shuffle broadcasts) was
-// written in round 2, parity green, and removed: in-kernel counters gave 8.3 k cycles per iteration against 6.7 k for this
-// one (priors 2.5 k vs 1.5 k, solve 3.3 k vs 3.3 k, record 1.1 k vs 0.85 k) - the chain of dependent fp64 operations
-// (~16 cycles each) is what costs, and shuffles and selects only lengthen it.
-// Warp-collective. `s` is the hypothesis' optimiser state (global or shared memory); `pre` = the range prior at
-// the candidate pose if it was computed already, else nullptr (computed here).
-__device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const double* sums /* smem, kNacc */, int lane,
-                                    const PriorRes* pre) {
+// Warp-collective (the ray-march runs on the whole warp); lane 0 returns the terms in registers.
+__device__ __forceinline__ void prior_terms(const PassArgs& A, const double* Rc, const double* Cc, int lane, double (&Hp)[21],
+                                            double (&gp)[6], double& costp, unsigned& fl) {
   const pilot_refine_params& P = A.prm;
-
   double rr = 0.0, Jr[6];
   const bool range_on = range_enabled(A);
   bool range_ok = false;
-  if (range_on) {
-    if (pre) {
-      range_ok = pre->ok != 0; rr = pre->r;
-      for (int i = 0; i < 6; ++i) Jr[i] = pre->J[i];
+  if (range_on) range_ok = range_prior(A, Rc, Cc, lane, rr, Jr);
+#pragma unroll
+  for (int i = 0; i < 21; ++i) Hp[i] = 0.0;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) gp[i] = 0.0;
+  costp = 0.0; fl = 0u;
+  if (lane != 0) return;
+  if (P.w_gravity > 0.f) {                                                   // Eq.(3)
+    double e[3], r[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      e[i] = Rc[3 * i] * A.pd.gw[0] + Rc[3 * i + 1] * A.pd.gw[1] + Rc[3 * i + 2] * A.pd.gw[2];
+      r[i] = e[i] - A.pd.gi[i];
+    }
+    double rho, drho;
+    robust_d(P.loss, r[0] * r[0] + r[1] * r[1] + r[2] * r[2], A.pd.gravity_scale, rho, drho);
+    const double wg = A.pd.w_gravity * drho;
+    // J = [0 | -[e]x]: J^T r = e x r, J^T J = |e|^2 I - e e^T
+    const double ee = e[0] * e[0] + e[1] * e[1] + e[2] * e[2];
+    gp[3] = wg * (e[1] * r[2] - e[2] * r[1]);
+    gp[4] = wg * (e[2] * r[0] - e[0] * r[2]);
+    gp[5] = wg * (e[0] * r[1] - e[1] * r[0]);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = a; b < 3; ++b) Hp[tri(3 + a, 3 + b)] = wg * ((a == b ? ee : 0.0) - e[a] * e[b]);
+    costp = A.pd.w_gravity * rho;
+  }
+  if (range_on) {                                                            // Eq.(5)-(6) / ray-march
+    if (range_ok) {
+      double rho, drho;
+      robust_d(P.loss, rr * rr, A.pd.range_scale, rho, drho);
+      const double wr = A.pd.w_range * drho;
+#pragma unroll
+      for (int a = 0; a < 6; ++a) {
+        const double wj = wr * Jr[a];
+        gp[a] += wj * rr;
+#pragma unroll
+        for (int b = a; b < 6; ++b) Hp[tri(a, b)] += wj * Jr[b];
+      }
+      costp += A.pd.w_range * rho;
     } else {
-      range_ok = range_prior(A, s.Rc, s.Cc, lane, rr, Jr);
+      fl |= PILOT_STATUS_RANGE_SKIP;
     }
   }
-  if (lane != 0) return;
+}
+
+// The same into memory (shared): what the resident kernel's prior warp calls.
+__device__ __forceinline__ void prior_terms_store(const PassArgs& A, const double* Rc, const double* Cc, int lane, PriorTerms* out) {
+  double Hp[21], gp[6], costp;
+  unsigned fl;
+  prior_terms(A, Rc, Cc, lane, Hp, gp, costp, fl);
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < 21; ++i) out->H[i] = Hp[i];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) out->g[i] = gp[i];
+    out->cost = costp; out->flags = fl;
+  }
+}
+
+// Lane 0 does everything after the warp-wide ray-march; what it runs is ONE chain of dependent fp64 operations (8 cycles
+// each on B200, and a DFMA occupies the issue slot for 2), so the code is written for few instructions and a short chain:
+// the accepted system goes to the solve in registers (not through the state), the priors arrive as 28 numbers to add.
+// A lane-parallel variant (component i of the system in lane i, the record stores and state copies spread over the lanes,
+// a 6x6 Cholesky by rows with shuffle broadcasts) was written in round 2, parity green, and removed: 8.3 k cycles per
+// iteration against 6.7 k for the serial one of that time (3.1 k after the rewrite above; 2.x k now) - shuffles and
+// selects only lengthen the chain.
+// Warp-collective. `s` is the hypothesis' optimiser state (shared memory); `sums` the photo sums in double (shared memory);
+// `pre` = the priors' terms at the candidate pose if they were computed already, else nullptr (computed here).
+__device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const double* sums /* smem, kNacc */, int lane,
+                                    const PriorTerms* pre) {
+  const pilot_refine_params& P = A.prm;
+
+  double Hn[21], gn[6], costn;
+  unsigned fl = 0;
+  if (pre) {
+    if (lane != 0) return;
+#pragma unroll
+    for (int i = 0; i < 21; ++i) Hn[i] = pre->H[i];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) gn[i] = pre->g[i];
+    costn = pre->cost; fl = pre->flags;
+  } else {
+    prior_terms(A, s.Rc, s.Cc, lane, Hn, gn, costn, fl);
+    if (lane != 0) return;
+  }
 #ifdef PILOT_FIN_PROFILE
   long long tp[6]; tp[0] = clock64();
 #define PILOT_TP(i) tp[i] = clock64();
 #else
 #define PILOT_TP(i)
 #endif
-
-  double Hn[21], gn[6], costn;
-  unsigned fl = 0;
-  for (int i = 0; i < 21; ++i) Hn[i] = sums[i];          // converted to double by the 32 lanes that summed them
-  for (int i = 0; i < 6; ++i) gn[i] = sums[21 + i];
-  costn = sums[27];
-  int nv = (int)(sums[28] + 0.5);
+#pragma unroll
+  for (int i = 0; i < 21; ++i) Hn[i] += sums[i];          // converted to double by the 32 lanes that summed them
+#pragma unroll
+  for (int i = 0; i < 6; ++i) gn[i] += sums[21 + i];
+  costn += sums[27];
+  const int nv = (int)(sums[28] + 0.5);
   s.visible_evals += (unsigned long long)nv;
   if (nv < P.min_valid) { costn = INFINITY; fl |= PILOT_STATUS_FEW_VALID; }
-
-  if (P.w_gravity > 0.f) {                                                   // Eq.(3)
-    double e[3], r[3];
-    for (int i = 0; i < 3; ++i) {
-      e[i] = s.Rc[3 * i] * (double)A.gw[0] + s.Rc[3 * i + 1] * (double)A.gw[1] + s.Rc[3 * i + 2] * (double)A.gw[2];
-      r[i] = e[i] - (double)A.gi[i];
-    }
-    double rho, drho;
-    robust_d(P.loss, r[0] * r[0] + r[1] * r[1] + r[2] * r[2], (double)P.gravity_scale, rho, drho);
-    double wg = (double)P.w_gravity * drho;
-    // J = [0 | -[e]x]; rows of -[e]x: (0, e2, -e1), (-e2, 0, e0), (e1, -e0, 0)
-    double Jg[3][3] = {{0, e[2], -e[1]}, {-e[2], 0, e[0]}, {e[1], -e[0], 0}};
-    for (int a = 0; a < 3; ++a) {
-      double ga = 0;
-      for (int i = 0; i < 3; ++i) ga += Jg[i][a] * r[i];
-      gn[3 + a] += wg * ga;
-      for (int b = a; b < 3; ++b) {
-        double h = 0;
-        for (int i = 0; i < 3; ++i) h += Jg[i][a] * Jg[i][b];
-        Hn[tri(3 + a, 3 + b)] += wg * h;
-      }
-    }
-    costn += (double)P.w_gravity * rho;
-  }
-  if (range_on) {                                                            // Eq.(5)-(6) / ray-march
-    if (range_ok) {
-      double rho, drho;
-      robust_d(P.loss, rr * rr, (double)P.range_scale, rho, drho);
-      double wr = (double)P.w_range * drho;
-      for (int a = 0; a < 6; ++a) {
-        gn[a] += wr * Jr[a] * rr;
-        for (int b = a; b < 6; ++b) Hn[tri(a, b)] += wr * Jr[a] * Jr[b];
-      }
-      costn += (double)P.w_range * rho;
-    } else {
-      fl |= PILOT_STATUS_RANGE_SKIP;
-    }
-  }
   if (isnan(costn)) s.status |= PILOT_STATUS_NONFINITE;
   PILOT_TP(1)
 
@@ -1384,36 +1440,60 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
   double lam = s.lambda;
   const bool first = s.pending == 0;
   if (first || P.lm_mode == PILOT_LM_FIXED || costn < s.cost) {
+#pragma unroll
     for (int i = 0; i < 9; ++i) s.R[i] = s.Rc[i];
+#pragma unroll
     for (int i = 0; i < 3; ++i) s.C[i] = s.Cc[i];
+#pragma unroll
     for (int i = 0; i < 21; ++i) s.H[i] = Hn[i];
+#pragma unroll
     for (int i = 0; i < 6; ++i) s.g[i] = gn[i];
     s.cost = costn; s.n_valid = nv; s.flags = fl;
-    if (!first && P.lm_mode == PILOT_LM_ADAPTIVE) lam = fmax(lam * (double)P.lambda_down, (double)P.lambda_min);
-  } else {
-    lam = fmin(lam * (double)P.lambda_up, (double)P.lambda_max);
+    if (!first && P.lm_mode == PILOT_LM_ADAPTIVE) lam = fmax(lam * A.pd.lambda_down, A.pd.lambda_min);
+  } else {                                                                   // the accepted state stays: the solve reads it back
+#pragma unroll
+    for (int i = 0; i < 21; ++i) Hn[i] = s.H[i];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) gn[i] = s.g[i];
+    costn = s.cost;
+    lam = fmin(lam * A.pd.lambda_up, A.pd.lambda_max);
   }
+  // from here on (Hn, gn, costn) = the ACCEPTED system, in registers for the first solve
 
   PILOT_TP(2)
   // record + damped solve (a9, Eq.8); a failed factorisation consumes the iteration and raises lambda
   bool have = false;
   const size_t Hn_ = (size_t)A.n_hyp;
-  while (s.k < A.iters) {
-    const size_t ri = (size_t)(A.rec_base + s.k) * Hn_ + (size_t)m;
+  int k = s.k;
+  bool again = false;
+  while (k < A.iters) {
+    if (again) {                                                             // cold: registers were given up after the first try
+#pragma unroll
+      for (int i = 0; i < 21; ++i) Hn[i] = s.H[i];
+#pragma unroll
+      for (int i = 0; i < 6; ++i) gn[i] = s.g[i];
+    }
+    again = true;
+    const size_t ri = (size_t)(A.rec_base + k) * Hn_ + (size_t)m;
     if (A.out.iter_hessian_dev) {
       float* o = A.out.iter_hessian_dev + 36 * ri;
+#pragma unroll
       for (int a = 0; a < 6; ++a)
-        for (int b = 0; b < 6; ++b) o[6 * a + b] = (float)s.H[a <= b ? tri(a, b) : tri(b, a)];
+#pragma unroll
+        for (int b = a; b < 6; ++b) { const float v = (float)Hn[tri(a, b)]; o[6 * a + b] = v; if (b != a) o[6 * b + a] = v; }
     }
-    if (A.out.iter_gradient_dev) for (int a = 0; a < 6; ++a) A.out.iter_gradient_dev[6 * ri + a] = (float)s.g[a];
-    if (A.out.iter_cost_dev) A.out.iter_cost_dev[ri] = (float)s.cost;
+    if (A.out.iter_gradient_dev)
+#pragma unroll
+      for (int a = 0; a < 6; ++a) A.out.iter_gradient_dev[6 * ri + a] = (float)gn[a];
+    if (A.out.iter_cost_dev) A.out.iter_cost_dev[ri] = (float)costn;
     if (A.out.iter_lambda_dev) A.out.iter_lambda_dev[ri] = (float)lam;
     double dxi[6];
     PILOT_TP(3)
-    bool ok = chol_solve6(s.H, lam, P.damp_mode, s.g, dxi);
+    const bool ok = chol_solve6(Hn, lam, P.damp_mode, gn, dxi, s.H, s.g);
     PILOT_TP(4)
-    s.k += 1;
+    k += 1;
     if (ok) {
+#pragma unroll
       for (int i = 0; i < 6; ++i) dxi[i] = -dxi[i];
       retract(s.R, s.C, dxi, s.Rc, s.Cc);                                    // Eq.(9)
       PILOT_TP(5)
@@ -1421,14 +1501,17 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
       have = true;
       break;
     }
-    if (lam >= (double)P.lambda_max) s.status |= PILOT_STATUS_CHOL_FAIL;
-    lam = fmin(lam * (double)P.lambda_up, (double)P.lambda_max);
+    if (lam >= A.pd.lambda_max) s.status |= PILOT_STATUS_CHOL_FAIL;
+    lam = fmin(lam * A.pd.lambda_up, A.pd.lambda_max);
   }
+  s.k = k;
   s.lambda = lam;
   if (!have) {                                                               // this level is finished
     s.level = A.level + 1;
-    s.k = 0; s.pending = 0; s.lambda = (double)P.lambda_init;
+    s.k = 0; s.pending = 0; s.lambda = A.pd.lambda_init;
+#pragma unroll
     for (int i = 0; i < 9; ++i) s.Rc[i] = s.R[i];
+#pragma unroll
     for (int i = 0; i < 3; ++i) s.Cc[i] = s.C[i];
     if (A.level + 1 == A.level_end) write_final(A, s, m);
   }

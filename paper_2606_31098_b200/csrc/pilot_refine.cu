@@ -399,6 +399,11 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
   A.prm = *p;
   for (int i = 0; i < 3; ++i) { A.gw[i] = in->gravity_world[i]; A.gi[i] = in->gravity_imu[i]; A.ray[i] = in->range_ray_cam[i]; }
   A.range_meas = in->range_meas;
+  A.pd.lambda_init = (double)p->lambda_init; A.pd.lambda_up = (double)p->lambda_up; A.pd.lambda_down = (double)p->lambda_down;
+  A.pd.lambda_min = (double)p->lambda_min; A.pd.lambda_max = (double)p->lambda_max;
+  A.pd.w_gravity = (double)p->w_gravity; A.pd.gravity_scale = (double)p->gravity_scale;
+  A.pd.w_range = (double)p->w_range; A.pd.range_scale = (double)p->range_scale;
+  for (int i = 0; i < 3; ++i) { A.pd.gw[i] = (double)in->gravity_world[i]; A.pd.gi[i] = (double)in->gravity_imu[i]; }
   A.dsm = in->dsm_dev; A.dsm_w = in->dsm_width; A.dsm_h = in->dsm_height;
   A.dsm_ox = in->dsm_origin_x; A.dsm_oy = in->dsm_origin_y; A.dsm_gsd = in->dsm_gsd;
   A.n_hyp = in->n_hypotheses; A.level_end = level_end;

@@ -8,8 +8,8 @@
 // shared memory in a fixed order (deterministic), adds the priors, takes the accept/reject decision, solves the
 // damped 6x6 system and retracts (finalize_hypothesis, shared with the pass kernel); a second cluster barrier
 // publishes the new candidate pose, which the other CTAs read from rank 0's shared memory. The heightfield
-// ray-march of the range prior depends only on the candidate pose, so one warp of the rank-0 CTA evaluates it
-// WHILE the other warps gather: it leaves the critical path. The optimiser state lives in shared memory for the
+// ray-march of the range prior and the algebra of both priors (their terms of supp Eq.5-6) depend only on the candidate
+// pose, so one warp of the rank-0 CTA evaluates them WHILE the other warps gather: they leave the critical path. The optimiser state lives in shared memory for the
 // whole level; launches, grid ramps, the atomic ticket and the global partial sums of the pass kernel disappear.
 //
 // Shares no code with oracle/.
@@ -31,7 +31,7 @@ struct ResidentShared {
   float part[kWarps][kNacc];
   float cta_sum[kNacc];              // this CTA's slice total; rank 0 reads it through DSMEM
   double tot[kNacc];                 // the cluster's sums, converted to double by the lane that added each
-  PriorRes prior;
+  PriorTerms prior;                  // what the priors add at the candidate pose (the prior warp writes it during the gather)
   int go;
 };
 
@@ -75,12 +75,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
 
     acc_zero<MMA>(acc, sacc);
     if (prior_warp) {
-      double rr = 0.0, Jr[6];
-      const bool ok = range_prior(A, sh.pose, sh.pose + 9, lane, rr, Jr);
-      if (lane == 0) {
-        sh.prior.ok = ok ? 1 : 0; sh.prior.r = rr;
-        for (int i = 0; i < 6; ++i) sh.prior.J[i] = ok ? Jr[i] : 0.0;
-      }
+      prior_terms_store(A, sh.pose, sh.pose + 9, lane, &sh.prior);
     } else {
       photo_accumulate<T, G, CEN, MMA>(A, sh.pose, sh.pose + 9, 0, N, worker, n_workers, acc, sacc, red);
     }
