@@ -4,13 +4,15 @@
 // One launch per pyramid LEVEL instead of one per EVAL pass: a thread-block cluster of S CTAs owns one hypothesis
 // for all of that level's LM iterations (hypotheses are independent, so clusters never wait on each other).
 // Per iteration: every CTA gathers its slice of the anchors (same photo_accumulate as the pass kernel), reduces it
-// to 32 floats in shared memory; after a cluster barrier the rank-0 CTA sums the S slices through distributed
-// shared memory in a fixed order (deterministic), adds the priors, takes the accept/reject decision, solves the
-// damped 6x6 system and retracts (finalize_hypothesis, shared with the pass kernel); a second cluster barrier
-// publishes the new candidate pose, which the other CTAs read from rank 0's shared memory. The heightfield
-// ray-march of the range prior and the algebra of both priors (their terms of supp Eq.5-6) depend only on the candidate
-// pose, so one warp of the rank-0 CTA evaluates them WHILE the other warps gather: they leave the critical path. The optimiser state lives in shared memory for the
-// whole level; launches, grid ramps, the atomic ticket and the global partial sums of the pass kernel disappear.
+// to 32 floats in shared memory and SENDS them to the rank-0 CTA (asynchronous DSMEM stores that complete on rank 0's
+// mbarrier); rank 0's warp 0 waits for the S slices, sums them in a fixed order (deterministic), adds the priors, takes
+// the accept/reject decision, solves the damped 6x6 system and retracts (finalize_hypothesis, shared with the pass
+// kernel), then sends the new candidate pose into every CTA's shared memory (again st.async onto each CTA's own
+// mbarrier). There is no cluster-wide barrier inside the loop: only the threads that need a hand-off wait for it.
+// The heightfield ray-march of the range prior and the algebra of both priors (their terms of supp Eq.5-6) depend only
+// on the candidate pose, so one warp of the rank-0 CTA evaluates them WHILE the other warps gather: they leave the
+// critical path. The optimiser state lives in shared memory for the whole level; launches, grid ramps, the atomic
+// ticket and the global partial sums of the pass kernel disappear.
 //
 // Shares no code with oracle/.
 #ifndef PILOT_MMA_SB
@@ -27,13 +29,65 @@ namespace {
 
 struct ResidentShared {
   HypState st;                       // rank 0: the hypothesis' optimiser state for the whole level
-  __align__(16) double pose[12];     // this CTA's copy of the candidate pose: Rc[9], Cc[3]
+  __align__(16) double pose[12];     // candidate pose Rc[9], Cc[3]: written into EVERY rank's copy by rank 0's finaliser (DSMEM)
+  long long go;                      // ditto (right behind the pose): 1 = evaluate this pose, 0 = the level is finished
   float part[kWarps][kNacc];
-  float cta_sum[kNacc];              // this CTA's slice total; rank 0 reads it through DSMEM
+  __align__(16) float slice[8][kNacc];   // rank 0: the slice totals of every rank, written by their owners (DSMEM)
   double tot[kNacc];                 // the cluster's sums, converted to double by the lane that added each
   PriorTerms prior;                  // what the priors add at the candidate pose (the prior warp writes it during the gather)
-  int go;
+  unsigned long long bar_pose;       // mbarrier, 104 bytes per phase: rank 0's finaliser has published pose and go
+  unsigned long long bar_sums;       // mbarrier of rank 0, S x 128 bytes per phase: every rank's slice total is in `slice`
 };
+constexpr unsigned kPoseBytes = 13 * 8, kSliceBytes = kNacc * 4;
+
+// ---- cluster hand-offs: asynchronous DSMEM stores that complete on the CONSUMER's mbarrier (st.async ...
+// mbarrier::complete_tx::bytes): the data and its arrival are one message, so the producer needs no fence and only the
+// threads that need the data wait. Measured (config 1 | config 3 | paper schedule, ms per step): two cluster.sync() per
+// iteration, every thread of every CTA arriving and waiting, 0.504 | 0.850 | 0.251; plain DSMEM stores + a remote
+// mbarrier.arrive.release.cluster (ptxas puts MEMBAR.ALL.GPU in front of it) 0.496 | 0.832 | 0.248; this 0.468 | 0.809 | 0.242.
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned map_rank(unsigned addr, unsigned rank) {
+  unsigned r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+// the local arrival of a phase: so many bytes of asynchronous stores are expected before it completes
+__device__ __forceinline__ void mbar_arm(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "PILOT_WAIT:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra PILOT_DONE;\n"
+      "bra PILOT_WAIT;\n"
+      "PILOT_DONE:\n"
+      "}\n" ::"r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void st_async(unsigned dst, unsigned long long v, unsigned bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];" ::"r"(dst), "l"(v), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void st_async(unsigned dst, unsigned v, unsigned bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(dst), "r"(v), "r"(bar) : "memory");
+}
+
+// Rank 0's finaliser publishes the candidate pose and the go flag: lane r sends them to rank r (13 x 8 bytes completing on
+// rank r's bar_pose). Call with the whole warp after a __syncwarp().
+__device__ __forceinline__ void publish_pose(ResidentShared& sh, unsigned S, int lane, int level) {
+  if ((unsigned)lane < S) {
+    const unsigned dst = map_rank(smem_addr(sh.pose), (unsigned)lane), bar = map_rank(smem_addr(&sh.bar_pose), (unsigned)lane);
+#pragma unroll
+    for (int i = 0; i < 9; ++i) st_async(dst + 8u * i, (unsigned long long)__double_as_longlong(sh.st.Rc[i]), bar);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) st_async(dst + 8u * (9 + i), (unsigned long long)__double_as_longlong(sh.st.Cc[i]), bar);
+    st_async(dst + 8u * 12, (unsigned long long)(sh.st.level == level ? 1 : 0), bar);
+  }
+}
 
 template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel(const __grid_constant__ PassArgs A) {
@@ -44,34 +98,43 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
   __shared__ ResidentShared sh;
   PILOT_DECLARE_ACC
 
+  if (threadIdx.x == 0) {
+    mbar_init(&sh.bar_pose, 1u);
+    mbar_init(&sh.bar_sums, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_arm(&sh.bar_pose, kPoseBytes);              // phase 0
+  }
   if (rank == 0) {
     const int* src = reinterpret_cast<const int*>(A.state + m);
     int* dst = reinterpret_cast<int*>(&sh.st);
     for (int i = threadIdx.x; i < (int)(sizeof(HypState) / 4); i += kThreads) dst[i] = src[i];
-    __syncthreads();
-    if (threadIdx.x == 0) sh.go = sh.st.level == A.level;
   }
-  const ResidentShared* master = cluster.map_shared_rank(&sh, 0);
+  __syncthreads();
+  cluster.sync();                                    // every CTA of the cluster runs and its barriers are initialised
+  if (rank == 0 && warp == 0) publish_pose(sh, S, lane, A.level);
   const bool range_on = range_enabled(A);
   const bool prior_warp = range_on && rank == 0 && warp == kWarps - 1;
   // the gathering warps of the whole cluster share the anchors: worker w of n_workers (rank 0's last warp evaluates the
-  // range prior instead) - contiguous equal ranges on the tensor-core path, 32-anchor batches round-robin on the FFMA2 path
+  // priors instead) - 32-anchor batches round-robin
   const int n_workers = (int)S * kWarps - (range_on ? 1 : 0);
   const int worker = (int)rank * kWarps + warp - ((range_on && rank > 0) ? 1 : 0);
   const int N = A.lv.N;
+  const unsigned slice_dst = map_rank(smem_addr(&sh.slice[rank][lane]), 0u);
+  const unsigned sums_bar = map_rank(smem_addr(&sh.bar_sums), 0u);
 
 #ifdef PILOT_RESIDENT_PROFILE
   long long t_eval = 0, t_fin = 0, t_red = 0, t_all = clock64(), t0 = 0, n_it = 0;
 #endif
-  for (;;) {
-    cluster.sync();                                  // rank 0's candidate pose and go flag are published
+  for (unsigned phase = 0;; phase ^= 1u) {
+    mbar_wait(&sh.bar_pose, phase);                  // rank 0's candidate pose and go flag are in this CTA's shared memory
 #ifdef PILOT_RESIDENT_PROFILE
     t0 = clock64();
 #endif
-    const int go = master->go;
-    if (threadIdx.x < 12) sh.pose[threadIdx.x] = threadIdx.x < 9 ? master->st.Rc[threadIdx.x] : master->st.Cc[threadIdx.x - 9];
-    __syncthreads();
-    if (!go) break;
+    if (!*(volatile long long*)&sh.go) break;
+    if (threadIdx.x == 0) {                          // arm the next phase of the hand-offs this CTA receives
+      mbar_arm(&sh.bar_pose, kPoseBytes);
+      if (rank == 0) mbar_arm(&sh.bar_sums, S * kSliceBytes);
+    }
 
     acc_zero<MMA>(acc, sacc);
     if (prior_warp) {
@@ -85,28 +148,27 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
 #endif
     sh.part[warp][lane] = wtot;
     __syncthreads();
-    if (warp == 0) {
+    if (warp != 0) continue;
+    {
       float t = 0.f;
 #pragma unroll
       for (int w = 0; w < kWarps; ++w) t += sh.part[w][lane];            // fixed order
-      sh.cta_sum[lane] = t;
+      st_async(slice_dst, __float_as_uint(t), sums_bar);
     }
-    cluster.sync();                                  // every slice total (and the prior) is in shared memory
+    if (rank != 0) continue;
+    mbar_wait(&sh.bar_sums, phase);                  // every slice total (and, through rank 0's __syncthreads, the priors)
 #ifdef PILOT_RESIDENT_PROFILE
     t_red += clock64() - t0; t0 = clock64(); ++n_it;
 #endif
-    if (rank == 0 && warp == 0) {
-      float v[8];
-#pragma unroll
-      for (unsigned r = 0; r < 8; ++r) v[r] = r < S ? cluster.map_shared_rank(&sh, r)->cta_sum[lane] : 0.f;   // loads in flight together
+    {
       float t = 0.f;
 #pragma unroll
-      for (unsigned r = 0; r < 8; ++r) t += v[r];                         // fixed order
+      for (unsigned r = 0; r < 8; ++r) t += r < S ? *(volatile float*)&sh.slice[r][lane] : 0.f;   // fixed order
       sh.tot[lane] = (double)t;
       __syncwarp();
       finalize_hypothesis(A, sh.st, m, sh.tot, lane, range_on ? &sh.prior : nullptr);
       __syncwarp();
-      if (lane == 0) sh.go = sh.st.level == A.level;
+      publish_pose(sh, S, lane, A.level);
 #ifdef PILOT_RESIDENT_PROFILE
       t_fin += clock64() - t0;
 #endif
@@ -119,11 +181,11 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel
   }
 #endif
   if (rank == 0) {                                   // the state goes back to the workspace for the next level
+    __syncthreads();
     const int* src = reinterpret_cast<const int*>(&sh.st);
     int* dst = reinterpret_cast<int*>(A.state + m);
     for (int i = threadIdx.x; i < (int)(sizeof(HypState) / 4); i += kThreads) dst[i] = src[i];
   }
-  cluster.sync();                                    // rank 0's shared memory outlives every remote read
 }
 
 typedef void (*resident_fn)(const PassArgs);
