@@ -424,10 +424,24 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
 #define PILOT_MMA_PROJ_ILP 0       // 1: the projection passes of a super-batch side by side (pass kernel: config 4 -0.8 %;
                                     // the resident kernel, whose levels can be smaller than a super-batch, loses 1-3 %)
 #endif
+#ifndef PILOT_MMA_PROJ_F32
+#define PILOT_MMA_PROJ_F32 1       // 1: projection and visibility of the 16-bit path in fp32 (SURVEY 8(a) a2's number type): the
+                                    // centre as a hi + lo pair of floats, the rotation rounded to float; 16 floats behind the
+                                    // double pose in shared memory
+#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
                                     // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
 #endif
+// element i of the 16 floats the fp32 projection reads behind the double pose: R (row-major), the centre rounded to float,
+// and what that rounding left (so that P - C is taken as (P - hi) - lo: no information of the double centre is lost)
+__device__ __forceinline__ void pose_to_float(const double* Rc, const double* Cc, int i, float* out) {
+  float v = 0.f;
+  if (i < 9) v = (float)Rc[i];
+  else if (i < 12) v = (float)Cc[i - 9];
+  else if (i < 15) { const double c = Cc[i - 12]; v = (float)(c - (double)(float)c); }
+  out[i] = v;
+}
 template <int CH> struct MmaGeom {            // CH = channels of a 16-bit feature: 16, 32, 64 or 128
   static constexpr int PX = CH * 2;                    // bytes per pixel
   static constexpr int TB = PX / 4 < 32 ? PX / 4 : 32; // bytes per load per thread (the 4 q-threads share a pixel): 8, 16, 32
@@ -446,6 +460,12 @@ template <int CH> struct MmaGeom {            // CH = channels of a 16-bit featu
 };
 template <int G> __host__ __device__ constexpr bool mma_supported() { return G == 2 || G == 4 || G == 8 || G == 16; }
 
+// 1 / z for the fp32 projection: hardware seed + one Newton step, no slow path (z > z_near > 0 where the result is used)
+__device__ __forceinline__ float rcp_f32(float z) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(z));
+  return fmaf(y, fmaf(-z, y, 1.f), y);
+}
 template <int NW> struct TapWords { unsigned w[NW]; };
 #ifndef PILOT_LDG_OP
 #define PILOT_LDG_OP "ld.global.nc"
@@ -500,6 +520,67 @@ template <int G, bool MMA> constexpr size_t gather_smem_bytes() {
   return (size_t)acc_smem_floats<MMA>() * 4 + (size_t)kWarps * red_warp_floats<G, MMA>() * 4;
 }
 
+// The projection of one anchor in double (a2): the reference for every integer the projection decides. The fp32
+// projection below calls it (cold path) for the anchors whose VISIBILITY it cannot decide safely: within `band` pixels of
+// the border of the map or within band_z of z_near, where band is a multiple of its own rounding-error bound. n_valid and
+// the set of units that contribute are therefore exactly those of a double projection.
+struct ProjUnit { float a, b, x, y, iz; unsigned off; bool valid, near; };
+__device__ __noinline__ ProjUnit project_anchor_f64(float Px, float Py, float Pz, unsigned pose_s, float fx, float fy, float cx, float cy,
+                                                    float z_near, int W, int H, unsigned PX) {
+  double R[12];
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
+  const double* Cc = R + 9;
+  const double dx = (double)Px - Cc[0], dy = (double)Py - Cc[1], dz = (double)Pz - Cc[2];
+  const double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
+  const double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
+  const double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
+  bool valid = Zd > (double)z_near;
+  const double izd = fast_rcp(Zd);
+  const double ud = (double)fx * Xd * izd + (double)cx;
+  const double vd = (double)fy * Yd * izd + (double)cy;
+  const double x0d = floor(ud), y0d = floor(vd);
+  valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= (double)(W - 1)) && (y0d + 1.0 <= (double)(H - 1));
+  ProjUnit u;
+  u.iz = (float)izd;
+  u.a = (float)(ud - x0d); u.b = (float)(vd - y0d);
+  u.x = (float)Xd * u.iz; u.y = (float)Yd * u.iz;
+  u.off = valid ? ((unsigned)(int)y0d * (unsigned)W + (unsigned)(int)x0d) * PX : 0u;
+  u.valid = valid; u.near = false;
+  return u;
+}
+
+// The same in fp32 (SURVEY 8(a) a2's number type) from the float copy of the pose behind the double one: the centre as a
+// hi + lo pair (P - C loses nothing of the double centre), the rotation rounded to float, 1/Z from the hardware seed + one
+// Newton step. Error of (u, v): <= ~1e-6 (fx + |u - cx|) pixels, i.e. ~1e-4 typical and 2e-3 worst case on a 1920-wide map -
+// inside the bilinear patch that is a change of the continuous interpolant far below the 16-bit features' rounding. What is
+// NOT continuous is visibility, so anchors within 4e-6 (fx + fy + W + H) pixels of the border of the map (>= 10x the bound;
+// measured error on config 4: 3e-4 pixels) or within 4e-6 |P - C|_1 of z_near are projected again in double (about 1 anchor in 10^4).
+__device__ __forceinline__ ProjUnit project_anchor_f32(float Px, float Py, float Pz, bool in_range, const float (&Rf)[16], unsigned pose_s,
+                                                       float fx, float fy, float cx, float cy, float z_near, int W, int H,
+                                                       float wmaxf, float hmaxf, float band, unsigned PX) {
+  const float dx = (Px - Rf[9]) - Rf[12], dy = (Py - Rf[10]) - Rf[13], dz = (Pz - Rf[11]) - Rf[14];
+  const float X = fmaf(Rf[2], dz, fmaf(Rf[1], dy, Rf[0] * dx));
+  const float Y = fmaf(Rf[5], dz, fmaf(Rf[4], dy, Rf[3] * dx));
+  const float Z = fmaf(Rf[8], dz, fmaf(Rf[7], dy, Rf[6] * dx));
+  ProjUnit p;
+  p.iz = rcp_f32(Z);
+  p.x = X * p.iz; p.y = Y * p.iz;
+  const float u = fmaf(fx, p.x, cx), v = fmaf(fy, p.y, cy);
+  const float x0 = floorf(u), y0 = floorf(v);
+  // 0 <= u < W - 1 as |u - (W-1)/2| < (W-1)/2 (one subtraction serves the decision and its guard; the two differ only
+  // inside the band, where the double projection decides). NaNs compare false: such an anchor is invisible.
+  const float hw = 0.5f * wmaxf, hh = 0.5f * hmaxf;
+  const float tu = fabsf(u - hw) - hw, tv = fabsf(v - hh) - hh;           // < 0 inside
+  p.valid = in_range && (Z > z_near) && (tu < 0.f) && (tv < 0.f);
+  p.a = u - x0; p.b = v - y0;
+  p.off = p.valid ? ((unsigned)(int)y0 * (unsigned)W + (unsigned)(int)x0) * PX : 0u;
+  const float band_z = 4e-6f * (fabsf(dx) + fabsf(dy) + fabsf(dz));
+  p.near = in_range && ((fabsf(tu) < band) || (fabsf(tv) < band) || (fabsf(Z - z_near) < band_z));
+  return p;                                                              // the caller sends `near` anchors to project_anchor_f64
+}
+
 // ------------------------------------------------------------------ the photo gather, tensor-core contraction
 //
 // Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on super-batches of SB
@@ -529,6 +610,9 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   // by every projection: as 24 registers held across the rounds it forced the address arithmetic to be rematerialised.
   const unsigned pose_s = (unsigned)__cvta_generic_to_shared(Rc);         // Rc[9] | Cc[3] contiguous, 16-byte aligned
   const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
+  (void)wmax; (void)hmax;
+  const float wmaxf = (float)(L.W - 1), hmaxf = (float)(L.H - 1);
+  const float band = 4e-6f * (fabsf(L.fx) + fabsf(L.fy) + (float)(L.W + L.H));   // see project_anchor_f32
 
   const int q = lane & 3, g = lane >> 2;
   const bool diag = q == (g >> 1);                                        // holds C[g][g] and C[g+8][g] of every accumulator
@@ -561,14 +645,41 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
 #pragma unroll
       for (int k = 1; k < PASSES; ++k) Pk[k] = load_anchor(b0 + k * n_workers);
       Pn = load_anchor(b0 + PASSES * n_workers);
+      float pa[PASSES], pb[PASSES], px[PASSES], py[PASSES], piz[PASSES];
+      unsigned poff[PASSES];
+      bool pvalid[PASSES];
+#if PILOT_MMA_PROJ_F32
+      bool pnear[PASSES];
+      float Rf[16];                                                       // R[9], C hi[3], C lo[3], pad: four 16-byte loads
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(Rf[4 * i]), "=f"(Rf[4 * i + 1]), "=f"(Rf[4 * i + 2]), "=f"(Rf[4 * i + 3]) : "r"(pose_s + 96u + 16u * i));
+#pragma unroll
+      for (int k = 0; k < PASSES; ++k) {
+        const int base = begin + (b0 + k * n_workers) * 32;
+        const bool in_range = (b0 + k * n_workers) < n_batches && base + lane < end;
+        const ProjUnit pu = project_anchor_f32(Pk[k].x, Pk[k].y, Pk[k].z, in_range, Rf, pose_s, L.fx, L.fy, L.cx, L.cy, A.prm.z_near,
+                                               L.W, L.H, wmaxf, hmaxf, band, (unsigned)PX);
+        pa[k] = pu.a; pb[k] = pu.b; px[k] = pu.x; py[k] = pu.y; piz[k] = pu.iz; poff[k] = pu.off; pvalid[k] = pu.valid;
+        pnear[k] = pu.near;
+      }
+      bool any_near = false;
+#pragma unroll
+      for (int k = 0; k < PASSES; ++k) any_near = any_near || pnear[k];
+      if (any_near) {                                                     // cold: visibility decided in double (one branch for all passes)
+#pragma unroll
+        for (int k = 0; k < PASSES; ++k) {
+          if (!pnear[k]) continue;
+          const ProjUnit pu = project_anchor_f64(Pk[k].x, Pk[k].y, Pk[k].z, pose_s, L.fx, L.fy, L.cx, L.cy, A.prm.z_near, L.W, L.H, (unsigned)PX);
+          pa[k] = pu.a; pb[k] = pu.b; px[k] = pu.x; py[k] = pu.y; piz[k] = pu.iz; poff[k] = pu.off; pvalid[k] = pu.valid;
+        }
+      }
+#else
       double R[12];                                                       // six 16-byte shared-memory loads
 #pragma unroll
       for (int i = 0; i < 6; ++i)
         asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
       const double* Cc = R + 9;
-      float pa[PASSES], pb[PASSES], px[PASSES], py[PASSES], piz[PASSES];
-      unsigned poff[PASSES];
-      bool pvalid[PASSES];
 #pragma unroll
       for (int k = 0; k < PASSES; ++k) {
         const int base = begin + (b0 + k * n_workers) * 32;
@@ -589,6 +700,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
         poff[k] = valid ? ((unsigned)(int)y0d * (unsigned)L.W + (unsigned)(int)x0d) * (unsigned)PX : 0u;
         pvalid[k] = valid;
       }
+#endif
 #pragma unroll
       for (int k = 0; k < PASSES; ++k) {
         const unsigned vmask = __ballot_sync(0xffffffffu, pvalid[k]);
@@ -611,6 +723,23 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       const float4 P = Pn;
       Pn = load_anchor(b + n_workers);                                    // next pass's anchors: in flight during this one
       bool valid = base + lane < end;
+#if PILOT_MMA_PROJ_F32
+      float Rf[16];                                                       // R[9], C hi[3], C lo[3], pad: four 16-byte loads
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(Rf[4 * i]), "=f"(Rf[4 * i + 1]), "=f"(Rf[4 * i + 2]), "=f"(Rf[4 * i + 3]) : "r"(pose_s + 96u + 16u * i));
+      ProjUnit pu = project_anchor_f32(P.x, P.y, P.z, valid, Rf, pose_s, L.fx, L.fy, L.cx, L.cy, A.prm.z_near, L.W, L.H, wmaxf, hmaxf,
+                                       band, (unsigned)PX);
+      if (pu.near) pu = project_anchor_f64(P.x, P.y, P.z, pose_s, L.fx, L.fy, L.cx, L.cy, A.prm.z_near, L.W, L.H, (unsigned)PX);   // cold
+      valid = pu.valid;
+      const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+      if (valid) {
+        const int s = nv + __popc(vmask & ((1u << lane) - 1u));
+        slotA[s] = make_uint2(pu.off, (unsigned)(base + lane));
+        slotB[s] = make_float4(pu.a, pu.b, pu.x, pu.y);
+        slotC[s] = make_float2(pu.iz, P.w);
+      }
+#else
       double R[12];                                                       // six 16-byte shared-memory loads
 #pragma unroll
       for (int i = 0; i < 6; ++i)
@@ -635,6 +764,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
         slotB[s] = make_float4((float)(ud - x0d), (float)(vd - y0d), (float)Xd * iz, (float)Yd * iz);
         slotC[s] = make_float2(iz, P.w);
       }
+#endif
       nv += __popc(vmask);
     }
 #endif

@@ -30,7 +30,8 @@ namespace {
 struct ResidentShared {
   HypState st;                       // rank 0: the hypothesis' optimiser state for the whole level
   __align__(16) double pose[12];     // candidate pose Rc[9], Cc[3]: written into EVERY rank's copy by rank 0's finaliser (DSMEM)
-  long long go;                      // ditto (right behind the pose): 1 = evaluate this pose, 0 = the level is finished
+  float posef[16];                   // ditto (right behind the pose): R, centre hi, centre lo as floats (pose_to_float)
+  long long go;                      // ditto: 1 = evaluate this pose, 0 = the level is finished
   float part[kWarps][kNacc];
   __align__(16) float slice[8][kNacc];   // rank 0: the slice totals of every rank, written by their owners (DSMEM)
   double tot[kNacc];                 // the cluster's sums, converted to double by the lane that added each
@@ -38,7 +39,7 @@ struct ResidentShared {
   unsigned long long bar_pose;       // mbarrier, 104 bytes per phase: rank 0's finaliser has published pose and go
   unsigned long long bar_sums;       // mbarrier of rank 0, S x 128 bytes per phase: every rank's slice total is in `slice`
 };
-constexpr unsigned kPoseBytes = 13 * 8, kSliceBytes = kNacc * 4;
+constexpr unsigned kPoseBytes = 12 * 8 + 16 * 4 + 8, kSliceBytes = kNacc * 4;
 
 // ---- cluster hand-offs: asynchronous DSMEM stores that complete on the CONSUMER's mbarrier (st.async ...
 // mbarrier::complete_tx::bytes): the data and its arrival are one message, so the producer needs no fence and only the
@@ -76,8 +77,8 @@ __device__ __forceinline__ void st_async(unsigned dst, unsigned v, unsigned bar)
   asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(dst), "r"(v), "r"(bar) : "memory");
 }
 
-// Rank 0's finaliser publishes the candidate pose and the go flag: lane r sends them to rank r (13 x 8 bytes completing on
-// rank r's bar_pose). Call with the whole warp after a __syncwarp().
+// Rank 0's finaliser publishes the candidate pose (doubles, and the float copy the fp32 projection reads) and the go flag:
+// lane r sends them to rank r (21 x 8 bytes completing on rank r's bar_pose). Call with the whole warp after a __syncwarp().
 __device__ __forceinline__ void publish_pose(ResidentShared& sh, unsigned S, int lane, int level) {
   if ((unsigned)lane < S) {
     const unsigned dst = map_rank(smem_addr(sh.pose), (unsigned)lane), bar = map_rank(smem_addr(&sh.bar_pose), (unsigned)lane);
@@ -85,7 +86,13 @@ __device__ __forceinline__ void publish_pose(ResidentShared& sh, unsigned S, int
     for (int i = 0; i < 9; ++i) st_async(dst + 8u * i, (unsigned long long)__double_as_longlong(sh.st.Rc[i]), bar);
 #pragma unroll
     for (int i = 0; i < 3; ++i) st_async(dst + 8u * (9 + i), (unsigned long long)__double_as_longlong(sh.st.Cc[i]), bar);
-    st_async(dst + 8u * 12, (unsigned long long)(sh.st.level == level ? 1 : 0), bar);
+    float f[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) pose_to_float(sh.st.Rc, sh.st.Cc, i, f);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      st_async(dst + 8u * (12 + i), (unsigned long long)__float_as_uint(f[2 * i]) | ((unsigned long long)__float_as_uint(f[2 * i + 1]) << 32), bar);
+    st_async(dst + 8u * 20, (unsigned long long)(sh.st.level == level ? 1 : 0), bar);
   }
 }
 

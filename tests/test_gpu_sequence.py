@@ -78,9 +78,16 @@ def test_config3_streaming_sequence():
         orc = oracle_frame(kept[i], seeds)
         g = dict(poses=poses, cost=cost)
         conv = parity.converged(orc, step_tol=5e-4)       # 200-400 m ranges: last accepted steps are ~1e-5..1e-4 m
-        assert conv.sum() >= seq.H // 2, (i, conv.sum())
         er, et = parity.pose_errors(g, orc)
+        # Whether the ORACLE ends a frame on a tiny accepted step depends on the seeds to the last bit (on some frames an
+        # anchor at the border of the map makes it reject every step after one of ~1e-3 m, for most hypotheses at once),
+        # and the seeds are the GPU's own estimate of the previous frame: the size of the flagged set is a property of
+        # the frame, not of the path under test. What is asserted: every flagged hypothesis agrees, the set is not empty,
+        # and at least half of ALL hypotheses agree with the oracle whatever it flagged ("report the
+        # matching fraction of the rest").
+        assert conv.any(), i
         assert er[conv].max() <= TOL and et[conv].max() <= TOL, (i, er[conv].max(), et[conv].max())
+        assert ((er <= TOL) & (et <= TOL)).sum() >= seq.H // 2, (i, ((er <= TOL) & (et <= TOL)).sum())
         b = ph.select_best(orc["cost64"])
         assert er[b] <= TOL and et[b] <= TOL
         gb = int(rows[i, 13])
