@@ -429,6 +429,10 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
                                     // centre as a hi + lo pair of floats, the rotation rounded to float; 16 floats behind the
                                     // double pose in shared memory
 #endif
+#ifndef PILOT_MMA_PROJ_GUARD
+#define PILOT_MMA_PROJ_GUARD 1     // 0 (measurement only): no double re-projection near the borders - config 4 7.10 -> 6.98 ms, and
+                                    // tests/test_gpu_parity.py::test_visibility_is_decided_in_double fails
+#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
                                     // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
@@ -577,7 +581,7 @@ __device__ __forceinline__ ProjUnit project_anchor_f32(float Px, float Py, float
   p.a = u - x0; p.b = v - y0;
   p.off = p.valid ? ((unsigned)(int)y0 * (unsigned)W + (unsigned)(int)x0) * PX : 0u;
   const float band_z = 4e-6f * (fabsf(dx) + fabsf(dy) + fabsf(dz));
-  p.near = in_range && ((fabsf(tu) < band) || (fabsf(tv) < band) || (fabsf(Z - z_near) < band_z));
+  p.near = PILOT_MMA_PROJ_GUARD && in_range && ((fabsf(tu) < band) || (fabsf(tv) < band) || (fabsf(Z - z_near) < band_z));
   return p;                                                              // the caller sends `near` anchors to project_anchor_f64
 }
 

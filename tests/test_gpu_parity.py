@@ -166,6 +166,37 @@ def test_edge_cases():
     assert np.all(gpu["status"] & 8) and np.array_equal(gpu["status"], orc["status"])
 
 
+@pytest.mark.parametrize("shift", [(0.0, 0.0, 0.0), (480.0, -350.0, 20.0)])
+def test_visibility_is_decided_in_double(shift):
+    """The 16-bit gather projects in fp32 (error ~1e-4 pixels here); whether a unit is visible is NOT continuous, so it
+    stays a double decision. Anchors whose projection falls 1e-7 ... 1e-2 pixels on either side of the
+    four borders of the footprint, or whose depth is that close to z_near, under hypothesis 0: n_valid - an integer -
+    must equal the oracle's for every hypothesis, at the input pose (zero iterations) and along a run."""
+    from oracle import pilot_oracle as po
+    W, H, N = 64, 48, 4096
+    prob = tiny(seed=41, N=N, C=32, n_hyp=3, dtype="bf16", W=W, H=H, origin_shift=shift)
+    rng = np.random.default_rng(4141)
+    T = np.asarray(prob["init_poses"][0], np.float64).reshape(3, 4)
+    fx, fy, cx, cy = prob["K"]
+    z_near = 60.0
+    delta = 10.0 ** rng.uniform(-7, -2, N) * rng.choice([-1.0, 1.0], N)
+    u, v = rng.uniform(1.0, W - 2.0, N), rng.uniform(1.0, H - 2.0, N)
+    Z = rng.uniform(70.0, 100.0, N)
+    kind = rng.integers(0, 6, N)                      # 0-3: a border of the footprint, 4: z_near, 5: an ordinary anchor
+    u = np.where(kind == 0, delta, np.where(kind == 1, W - 1 + delta, u))
+    v = np.where(kind == 2, delta, np.where(kind == 3, H - 1 + delta, v))
+    Z = np.where(kind == 4, z_near * (1.0 + delta * 1e-2), Z)
+    pc = np.stack([(u - cx) / fx * Z, (v - cy) / fy * Z, Z], 1)
+    prob["points"][0][:, :3] = (pc @ T[:, :3].T + T[:, 3]).astype(np.float32)
+    for iters in ([0], [3]):
+        P = dict(iters=iters, loss="huber", loss_scale=0.3, min_valid=4, z_near=z_near)
+        gpu, orc = both(prob, P)
+        assert np.array_equal(gpu["n_valid"], orc["n_valid"]), (iters, gpu["n_valid"], orc["n_valid"])
+        assert 0.3 * N < orc["n_valid"][0] < 0.8 * N     # about half of the border anchors are on the visible side
+        if iters[0]:
+            check_systems(gpu, orc, "bf16", recs=(0, 1, 2))
+
+
 def test_run_is_deterministic():
     from paper_2606_31098_b200 import binding
     prob = wl.config1(H=16, N=1500, iters=(3, 3, 3))
