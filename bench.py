@@ -27,7 +27,7 @@ LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", 
 # captures of this command (profiles/<file>): the first EVAL pass of a timed step (hypotheses spread over their initial
 # poses: the union of their footprints covers the map) and a late pass (hypotheses converged onto one pose). None where
 # no capture of that workload exists. Labelled with their source; everything else in the line is measured in this run.
-NCU_TRAFFIC = {"config4": {"first_pass_bytes": 422.0e6, "converged_pass_bytes": 31.5e6,
+NCU_TRAFFIC = {"config4": {"first_pass_bytes": 429.0e6, "converged_pass_bytes": 31.5e6,
                            "source": "profiles/r2_photo_config4.md"}}
 
 
@@ -556,8 +556,10 @@ def dtype_string(W):
     d = W.prob["dtype"]
     if d == "f32":
         return "f32"
-    return d + (" storage; first differences in %s, products on mma.sync with f32 accumulate" % d if mma else " storage, f32 FFMA2 contraction") + \
-        "; f32 lift, f64 projection and 6x6 solve"
+    if mma:
+        return d + (" storage; first differences in %s, products on mma.sync with f32 accumulate" % d) + \
+            "; f32 projection (visibility decided in f64) and lift, f64 6x6 solve"
+    return d + " storage, f32 FFMA2 contraction; f32 lift, f64 projection and 6x6 solve"
 
 
 def run_workload(name, args, rank, local_rank, world, use_dist, stream, steps, peaks, hbm, l2_bytes, with_e2e, with_cpu):

@@ -246,7 +246,12 @@ int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster);
  * 16, 32, 64 or 128 channels and the exact bilinear gradient, the first differences of the taps are taken in the
  * storage type (exact for neighbouring values within a factor of two; else one rounding of 2^-9 / 2^-12 relative to
  * the difference), and their 4 x 4 Gram matrix per unit is accumulated in fp32 on the tensor cores (mma.sync
- * m16n8k16); the bilinear combination follows in fp32. AUTO (default) = MMA where it applies AND was measured faster
+ * m16n8k16); the bilinear combination follows in fp32. This path also PROJECTS in fp32 (the camera
+ * centre as a hi + lo pair of floats, so P - C loses nothing of the double pose): (u, v) within ~1e-6 (fx + |u - cx|)
+ * pixels of the double projection, a change of the continuous bilinear interpolant far below the features' own rounding.
+ * Visibility is not continuous, so it stays a double decision: an anchor within 4e-6 (fx + fy + W + H) pixels of the
+ * border of the map, or within 4e-6 |P - C| of z_near, is projected again in double (n_valid and the set of
+ * contributing units are those of the double projection; FP32 projects every anchor in double). AUTO (default) = MMA where it applies AND was measured faster
  * (64 or more channels on the one-launch-per-pass strategy), FP32 elsewhere. Asking for MMA where it does not apply
  * falls back to FP32 (not an error). Results agree within the bf16 / fp16 parity
  * tolerance of the path (5e-3 relative on H and g); fp32 features always use FP32.
