@@ -241,6 +241,16 @@ typedef enum { PILOT_EXEC_AUTO = 0, PILOT_EXEC_PASSES = 1, PILOT_EXEC_RESIDENT =
 int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster);
 
 /*
+ * Optional extra records of the following runs on this handle (NULL = off, the default), for the backward pass of the
+ * unrolled refinement (pilot_refine_unrolled_backward): iter_poses_dev [sum(iters)][H][12] fp32 = the pose [R_wc | C] at
+ * which each recorded system (outputs.iter_hessian_dev ...) was built, i.e. the accepted pose at that solve;
+ * iter_accept_dev [sum(iters)][H] = 1 if the step solved from that record was accepted (PILOT_LM_FIXED: always), 0 if it
+ * was rejected or its factorisation failed (the pose did not move). Caller-owned device buffers, written in stream order
+ * by pilot_refine_run / run_levels (every launch strategy); rows of levels outside a run_levels range are untouched.
+ */
+int pilot_refine_set_iterate_outputs(pilot_refine_handle* h, float* iter_poses_dev, int* iter_accept_dev);
+
+/*
  * Arithmetic of the per-unit contraction (Eq.(1),(8) PAPER.md:118,160-164). FP32: taps are
  * unpacked to fp32 and every step runs on the FMA pipe (packed FFMA2). MMA: for 16-bit features (bf16 / fp16) with
  * 16, 32, 64 or 128 channels and the exact bilinear gradient, the first differences of the taps are taken in the
@@ -446,7 +456,7 @@ int pilot_refine_lift_anchors(const float* corners_dev, int crop_width, int crop
  * ground-truth projection lies inside [0, width-1] x [0, height-1]; the optimised projection may leave the image.
  * loss_dev[n_poses] (0 where V is empty), n_visible_dev[n_poses] = |V| (may be NULL). Projections, the loss and the
  * sums are double precision, summed in a fixed order. Asynchronous on cuda_stream, no allocation. The backward pass
- * through the unrolled LM steps is not part of this library.
+ * through the unrolled LM steps is pilot_refine_unrolled_backward below.
  * Errors: PILOT_ERR_ARG (NULL / misaligned pointer, scale <= 0, alpha NaN or +inf, bad image size), PILOT_ERR_CUDA.
  */
 int pilot_refine_reprojection_loss(const float* poses_dev, int n_poses, const float pose_star[12],
@@ -497,6 +507,59 @@ int pilot_refine_photo_backward(const void* query_feat_dev, const float* query_c
                                 const float* grad_hessian_dev, const float* grad_gradient_dev, int n_poses,
                                 pilot_loss loss, float loss_scale, float z_near, float* grad_feat_dev, float* grad_ref_dev,
                                 float* grad_conf_dev, float* grad_pose_dev, void* cuda_stream);
+
+/*
+ * Backward pass through ALL the LM steps of an unrolled refinement (supp III-C: "the
+ * refinement is unrolled over nine coarse-to-fine steps, and the final training objective averages the reprojection losses
+ * over all unrolled steps"). With T = sum(iters) solves, T^r the pose after r solves (T^0 = the initial pose) and
+ *   L = sum_{r=1..T} step_weights[r-1] L_r(T^r)        (L_r of supp Eq.8 as in pilot_refine_reprojection_loss; the paper's
+ *                                                       objective is step_weights = 1/T),
+ * it reads the chain  T^{r+1} = exp(dxi_r^) T^r (Eq.9), dxi_r = -(H_r + lambda_r D)^-1 g_r (Eq.8), (H_r, g_r) = the photo
+ * term at T^r on the level of solve r  backwards from the last pose - lm_step_adjoint, then photo_backward, per ACCEPTED
+ * solve; a rejected solve (or a failed factorisation) did not move the pose and passes dL/d eps through - and ADDS
+ *   grads.grad_feat_dev[l] [height_l][width_l][channels_l] fp32   dL/dF_l     (query feature map of level l)
+ *   grads.grad_ref_dev[l]  [n_points_l][channels_l]        fp32   dL/df^r_l
+ *   grads.grad_conf_dev[l] [height_l][width_l]             fp32   dL/dconf_l  (only where the level has a confidence map)
+ * (caller zeroes or pre-loads; any may be NULL) and WRITES grads.grad_init_pose_dev [H][6] = dL/d eps at the initial pose
+ * (left perturbation of T_cw, eps = (rho; phi)) and grads.loss_dev [H] = L (either may be NULL). One chain per hypothesis,
+ * all H side by side. lambda_r and the accept / reject decisions are piecewise constant and held fixed, as are the visible
+ * sets and bilinear cells. records: what a forward run with pilot_refine_set_iterate_outputs wrote (device pointers;
+ * final_poses_dev = outputs.poses_dev). `in`, `p`, cfg (level shapes and dtype) as given to that run. supervision: HOST
+ * scalars + the device points of V's candidates (pilot_refine_reprojection_loss); step_weights is a HOST array of T floats.
+ * The objective must be the photo term alone: PILOT_ERR_UNSUPPORTED if w_gravity != 0, the range prior is on, or grad_mode
+ * is not GRAD_BILINEAR_EXACT (the priors' pose-dependence is not part of this chain). scratch_dev: 256-byte aligned,
+ * at least pilot_refine_unrolled_backward_scratch_bytes(H, T) (else PILOT_ERR_WORKSPACE); no allocation. Asynchronous on
+ * cuda_stream: 4 launches per solve.
+ */
+typedef struct {
+  const float* iter_hessian_dev;    /* [T][H][36] */
+  const float* iter_gradient_dev;   /* [T][H][6]  */
+  const float* iter_lambda_dev;     /* [T][H]     */
+  const float* iter_poses_dev;      /* [T][H][12]  (pilot_refine_set_iterate_outputs) */
+  const int*   iter_accept_dev;     /* [T][H]      (pilot_refine_set_iterate_outputs) */
+  const float* final_poses_dev;     /* [H][12]     (outputs.poses_dev) */
+} pilot_refine_unrolled_records;
+typedef struct {
+  float pose_star[12];              /* ground-truth pose [R_wc | C] */
+  const float* points_dev;          /* [n_points][4] sampled 3-D points (16-byte aligned) */
+  int n_points;
+  float intrinsics[4];              /* K^q of supp Eq.7 */
+  int width, height;                /* image size that defines V */
+  float alpha, scale;               /* Barron loss shape and scale */
+  const float* step_weights;        /* HOST [T] */
+} pilot_refine_supervision;
+typedef struct {
+  float* grad_feat_dev[PILOT_MAX_LEVELS];
+  float* grad_ref_dev[PILOT_MAX_LEVELS];
+  float* grad_conf_dev[PILOT_MAX_LEVELS];
+  float* grad_init_pose_dev;        /* [H][6] */
+  float* loss_dev;                  /* [H] */
+} pilot_refine_unrolled_grads;
+size_t pilot_refine_unrolled_backward_scratch_bytes(int n_hypotheses, int total_iters);
+int pilot_refine_unrolled_backward(const pilot_refine_config* cfg, const pilot_refine_inputs* in, const pilot_refine_params* p,
+                                   const pilot_refine_unrolled_records* records, const pilot_refine_supervision* supervision,
+                                   const pilot_refine_unrolled_grads* grads, void* scratch_dev, size_t scratch_bytes,
+                                   void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Anchor order (kernel description PAPER.md:485). The sums of Eq.(2) and Eq.(8) do not depend on the

@@ -34,6 +34,7 @@ EXPORTS = ["pilot_refine_workspace_bytes", "pilot_refine_create", "pilot_refine_
            "pilot_refine_sequence_step", "pilot_refine_sequence_results", "pilot_refine_sequence_last_frame",
            "pilot_refine_sequence_last_launches", "pilot_refine_sequence_destroy", "pilot_refine_probe_gather",
            "pilot_refine_probe_unit_gather", "pilot_refine_last_visible_evals", "pilot_refine_last_plan",
+           "pilot_refine_set_iterate_outputs", "pilot_refine_unrolled_backward", "pilot_refine_unrolled_backward_scratch_bytes",
            "pilot_refine_sort_anchors", "pilot_refine_sort_anchors_temp_bytes",
            "pilot_refine_set_grid_host", "pilot_refine_submit_pruned_host",
            "pilot_refine_reprojection_loss_grad", "pilot_refine_lm_step_adjoint", "pilot_refine_photo_backward",
@@ -78,6 +79,22 @@ class Outputs(C.Structure):
                 ("status_dev", C.c_void_p), ("iter_hessian_dev", C.c_void_p),
                 ("iter_gradient_dev", C.c_void_p), ("iter_cost_dev", C.c_void_p),
                 ("iter_lambda_dev", C.c_void_p)]
+
+
+class UnrolledRecords(C.Structure):
+    _fields_ = [("iter_hessian_dev", C.c_void_p), ("iter_gradient_dev", C.c_void_p), ("iter_lambda_dev", C.c_void_p),
+                ("iter_poses_dev", C.c_void_p), ("iter_accept_dev", C.c_void_p), ("final_poses_dev", C.c_void_p)]
+
+
+class Supervision(C.Structure):
+    _fields_ = [("pose_star", C.c_float * 12), ("points_dev", C.c_void_p), ("n_points", C.c_int),
+                ("intrinsics", C.c_float * 4), ("width", C.c_int), ("height", C.c_int),
+                ("alpha", C.c_float), ("scale", C.c_float), ("step_weights", C.POINTER(C.c_float))]
+
+
+class UnrolledGrads(C.Structure):
+    _fields_ = [("grad_feat_dev", C.c_void_p * MAX_LEVELS), ("grad_ref_dev", C.c_void_p * MAX_LEVELS),
+                ("grad_conf_dev", C.c_void_p * MAX_LEVELS), ("grad_init_pose_dev", C.c_void_p), ("loss_dev", C.c_void_p)]
 
 
 class SequenceConfig(C.Structure):
@@ -198,6 +215,13 @@ def lib():
                                                   C.c_int, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                                   C.c_void_p]
         L.pilot_refine_photo_backward.restype = C.c_int
+        L.pilot_refine_set_iterate_outputs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.pilot_refine_set_iterate_outputs.restype = C.c_int
+        L.pilot_refine_unrolled_backward_scratch_bytes.argtypes = [C.c_int, C.c_int]
+        L.pilot_refine_unrolled_backward_scratch_bytes.restype = C.c_size_t
+        L.pilot_refine_unrolled_backward.argtypes = [C.POINTER(Config), C.POINTER(Inputs), C.POINTER(Params), C.POINTER(UnrolledRecords),
+                                                     C.POINTER(Supervision), C.POINTER(UnrolledGrads), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.pilot_refine_unrolled_backward.restype = C.c_int
         L.pilot_refine_set_grid_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.pilot_refine_set_grid_host.restype = C.c_int
         L.pilot_refine_submit_pruned_host.argtypes = [C.c_void_p, C.POINTER(Inputs), C.POINTER(Params), C.c_void_p, C.c_int,
@@ -405,6 +429,20 @@ class Refiner:
     def set_math_mode(self, math="auto"):
         _check(lib().pilot_refine_set_math_mode(self.handle, MATH_CODE[math]), "pilot_refine_set_math_mode")
 
+    def record_iterates(self, on=True):
+        """pilot_refine_set_iterate_outputs: the following runs also write, per solve, the pose the recorded system was built
+        at (iter_poses [T, H, 12]) and whether its step was accepted (iter_accept [T, H] int32); run() returns them."""
+        torch = self.torch
+        if on and "iter_poses" not in self.o:
+            H, T = self.o["poses"].shape[0], self.o["iter_cost"].numel() // self.o["poses"].shape[0]
+            dev = self.o["poses"].device
+            self.o["iter_poses"] = torch.zeros(T * H * 12, dtype=torch.float32, device=dev)
+            self.o["iter_accept"] = torch.zeros(T * H, dtype=torch.int32, device=dev)
+        self._iterates = bool(on)
+        _check(lib().pilot_refine_set_iterate_outputs(self.handle, self.o["iter_poses"].data_ptr() if on else None,
+                                                      self.o["iter_accept"].data_ptr() if on else None),
+               "pilot_refine_set_iterate_outputs")
+
     def set_chunk(self, chunk):
         _check(lib().pilot_refine_set_chunk(self.handle, int(chunk)), "pilot_refine_set_chunk")
 
@@ -437,6 +475,9 @@ class Refiner:
             elif name in ("iter_cost", "iter_lambda"): t = t[:T * H].view(T, H)
             else: t = t[:H]
             res[name] = t
+        if getattr(self, "_iterates", False):
+            res["iter_poses"] = self.o["iter_poses"][:T * H * 12].view(T, H, 12)
+            res["iter_accept"] = self.o["iter_accept"][:T * H].view(T, H)
         return res
 
     @property
@@ -485,6 +526,53 @@ def refine(prob, params=None, device=0, mode="auto", cluster=0, math="auto"):
     res["status"] = res["status"].view(np.uint32)
     res["launches"] = r.last_launches
     r.close()
+    return res
+
+
+def unrolled_backward(refiner, di, params, run_out, pose_star, sup_points, sup_intrinsics, width, height, alpha, scale,
+                      step_weights=None, grad_conf=False, stream=None):
+    """pilot_refine_unrolled_backward: the backward pass through every LM step of the run that produced `run_out` (the dict
+    Refiner.run returned with record_iterates() on). L = sum_r step_weights[r-1] L_r(pose after r solves); default weights
+    1/T (the paper's average over the unrolled steps). Returns dict: grad_feat / grad_ref (/ grad_conf) lists per level
+    (cuda fp32 tensors), grad_init_pose [H, 6], loss [H]. Marshalling only."""
+    torch = _torch()
+    par, P = make_params(params, di.n_levels)
+    H, T = di.n_hyp, sum(P["iters"])
+    dev = run_out["poses"].device
+    rec = UnrolledRecords()
+    rec.iter_hessian_dev, rec.iter_gradient_dev = run_out["iter_hessian"].data_ptr(), run_out["iter_gradient"].data_ptr()
+    rec.iter_lambda_dev = run_out["iter_lambda"].data_ptr()
+    rec.iter_poses_dev, rec.iter_accept_dev = run_out["iter_poses"].data_ptr(), run_out["iter_accept"].data_ptr()
+    rec.final_poses_dev = run_out["poses"].data_ptr()
+    w = np.full(max(T, 1), 1.0 / max(T, 1), np.float32) if step_weights is None else np.ascontiguousarray(step_weights, np.float32)
+    assert w.size >= T
+    sup = Supervision()
+    for i, v in enumerate(np.asarray(pose_star, np.float32).reshape(-1)):
+        sup.pose_star[i] = float(v)
+    sup.points_dev, sup.n_points = sup_points.data_ptr(), int(sup_points.shape[0])
+    for i in range(4):
+        sup.intrinsics[i] = float(sup_intrinsics[i])
+    sup.width, sup.height, sup.alpha, sup.scale = int(width), int(height), float(alpha), float(scale)
+    sup.step_weights = w.ctypes.data_as(C.POINTER(C.c_float))
+    g = UnrolledGrads()
+    res = dict(grad_feat=[], grad_ref=[], grad_conf=[])
+    for l in range(di.n_levels):
+        gf = torch.zeros(di.height[l], di.width[l], di.channels[l], dtype=torch.float32, device=dev)
+        gr = torch.zeros(int(di.inp.n_points[l]), di.channels[l], dtype=torch.float32, device=dev)
+        gc = torch.zeros(di.height[l], di.width[l], dtype=torch.float32, device=dev) if (grad_conf and di.inp.query_conf_dev[l]) else None
+        g.grad_feat_dev[l], g.grad_ref_dev[l] = gf.data_ptr(), gr.data_ptr()
+        g.grad_conf_dev[l] = gc.data_ptr() if gc is not None else None
+        res["grad_feat"].append(gf); res["grad_ref"].append(gr); res["grad_conf"].append(gc)
+    res["grad_init_pose"] = torch.zeros(H, 6, dtype=torch.float32, device=dev)
+    res["loss"] = torch.zeros(H, dtype=torch.float32, device=dev)
+    g.grad_init_pose_dev, g.loss_dev = res["grad_init_pose"].data_ptr(), res["loss"].data_ptr()
+    nb = lib().pilot_refine_unrolled_backward_scratch_bytes(H, T)
+    scratch = torch.empty(nb + 256, dtype=torch.uint8, device=dev)
+    sptr = (scratch.data_ptr() + 255) // 256 * 256
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    _check(lib().pilot_refine_unrolled_backward(C.byref(refiner.cfg), C.byref(di.inp), C.byref(par), C.byref(rec), C.byref(sup),
+                                                C.byref(g), sptr, nb, C.c_void_p(st.cuda_stream)), "pilot_refine_unrolled_backward")
+    st.synchronize()                               # scratch and the host weights may go
     return res
 
 

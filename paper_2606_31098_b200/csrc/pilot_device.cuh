@@ -90,6 +90,9 @@ struct PassArgs {
   float* partials;          // [n_hyp][n_chunks][kNacc]
   unsigned* counters;       // [n_hyp]
   pilot_refine_outputs out;
+  // optional extra records (pilot_refine_set_iterate_outputs; NULL = off)
+  float* iter_poses;        // [sum(iters)][n_hyp][12]: the accepted pose [R_wc | C] each recorded system was built at
+  int* iter_accept;         // [sum(iters)][n_hyp]: 1 if the step solved from that record was accepted
 };
 
 // pilot_resident.cu: one launch of the cluster-resident LM kernel for the level described by A (A.lv, A.level,
@@ -1584,6 +1587,7 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
     for (int i = 0; i < 6; ++i) s.g[i] = gn[i];
     s.cost = costn; s.n_valid = nv; s.flags = fl;
     if (!first && P.lm_mode == PILOT_LM_ADAPTIVE) lam = fmax(lam * A.pd.lambda_down, A.pd.lambda_min);
+    if (!first && A.iter_accept) A.iter_accept[(size_t)(A.rec_base + s.k - 1) * (size_t)A.n_hyp + (size_t)m] = 1;   // the step of record k - 1
   } else {                                                                   // the accepted state stays: the solve reads it back
 #pragma unroll
     for (int i = 0; i < 21; ++i) Hn[i] = s.H[i];
@@ -1621,6 +1625,14 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
       for (int a = 0; a < 6; ++a) A.out.iter_gradient_dev[6 * ri + a] = (float)gn[a];
     if (A.out.iter_cost_dev) A.out.iter_cost_dev[ri] = (float)costn;
     if (A.out.iter_lambda_dev) A.out.iter_lambda_dev[ri] = (float)lam;
+    if (A.iter_accept) A.iter_accept[ri] = 0;                                // set when (if) this record's step is accepted
+    if (A.iter_poses) {
+      float* T = A.iter_poses + 12 * ri;
+      for (int i = 0; i < 3; ++i) {
+        for (int c = 0; c < 3; ++c) T[4 * i + c] = (float)s.R[3 * c + i];    // R_wc = R_cw^T
+        T[4 * i + 3] = (float)s.C[i];
+      }
+    }
     double dxi[6];
     PILOT_TP(3)
     const bool ok = chol_solve6(Hn, lam, P.damp_mode, gn, dxi, s.H, s.g);

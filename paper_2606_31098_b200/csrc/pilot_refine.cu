@@ -92,7 +92,8 @@ struct pilot_refine_handle {
   int sm_count;
   int last_launches;
   int last_n_hyp;
-  unsigned last_mma_levels, last_resident_levels;   // bit l: level l of the last run used the tensor-core contraction / the resident kernel
+  unsigned last_mma_levels, last_resident_levels;
+  float* iter_poses; int* iter_accept;      // optional extra records (pilot_refine_set_iterate_outputs)   // bit l: level l of the last run used the tensor-core contraction / the resident kernel
   // host-path staging (create_host only)
   bool host_mode;
   int max_dsm_w, max_dsm_h;
@@ -267,6 +268,7 @@ int pilot_refine_create(const pilot_refine_config* cfg, pilot_refine_handle** ou
   h->last_launches = 0;
   h->last_n_hyp = 0;
   h->last_mma_levels = h->last_resident_levels = 0u;
+  h->iter_poses = nullptr; h->iter_accept = nullptr;
   h->host_mode = false; h->stage = nullptr; h->stage_bytes = 0; h->max_dsm_w = h->max_dsm_h = 0;
   h->copy_stream = nullptr; h->n_submitted = h->n_waited = 0;
   h->grid = nullptr; h->grid_n = 0;
@@ -320,6 +322,12 @@ int pilot_refine_set_exec_mode(pilot_refine_handle* h, int mode, int cluster) {
   if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return PILOT_ERR_ARG;
   h->mode = mode;
   h->cluster_override = cluster;
+  return PILOT_OK;
+}
+
+int pilot_refine_set_iterate_outputs(pilot_refine_handle* h, float* iter_poses_dev, int* iter_accept_dev) {
+  if (!h) return PILOT_ERR_ARG;
+  h->iter_poses = iter_poses_dev; h->iter_accept = iter_accept_dev;
   return PILOT_OK;
 }
 
@@ -411,6 +419,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
   A.counters = reinterpret_cast<unsigned*>(h->ws + w.counters);
   A.partials = reinterpret_cast<float*>(h->ws + w.partials);
   A.out = *out;
+  A.iter_poses = h->iter_poses; A.iter_accept = h->iter_accept;
 
   int launches = 0;
   unsigned plan_mma = 0u, plan_res = 0u;
