@@ -432,10 +432,6 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
                                     // centre as a hi + lo pair of floats, the rotation rounded to float; 16 floats behind the
                                     // double pose in shared memory
 #endif
-#ifndef PILOT_MMA_PROJ_GUARD
-#define PILOT_MMA_PROJ_GUARD 1     // 0 (measurement only): no double re-projection near the borders - config 4 7.10 -> 6.98 ms, and
-                                    // tests/test_gpu_parity.py::test_visibility_is_decided_in_double fails
-#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
                                     // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
@@ -474,9 +470,7 @@ __device__ __forceinline__ float rcp_f32(float z) {
   return fmaf(y, fmaf(-z, y, 1.f), y);
 }
 template <int NW> struct TapWords { unsigned w[NW]; };
-#ifndef PILOT_LDG_OP
-#define PILOT_LDG_OP "ld.global.nc"
-#endif
+#define PILOT_LDG_OP "ld.global.nc"    // (.cg, .cv, .lu, .ca, L1::no_allocate, L1::evict_first measured: no difference)
 template <int NW> __device__ __forceinline__ TapWords<NW> ldg_words(const char* p) {
   TapWords<NW> t;
   if constexpr (NW == 8) {                     // 32-byte load (sm_100: LDG.256); p is 32-byte aligned
@@ -584,7 +578,7 @@ __device__ __forceinline__ ProjUnit project_anchor_f32(float Px, float Py, float
   p.a = u - x0; p.b = v - y0;
   p.off = p.valid ? ((unsigned)(int)y0 * (unsigned)W + (unsigned)(int)x0) * PX : 0u;
   const float band_z = 4e-6f * (fabsf(dx) + fabsf(dy) + fabsf(dz));
-  p.near = PILOT_MMA_PROJ_GUARD && in_range && ((fabsf(tu) < band) || (fabsf(tv) < band) || (fabsf(Z - z_near) < band_z));
+  p.near = in_range && ((fabsf(tu) < band) || (fabsf(tv) < band) || (fabsf(Z - z_near) < band_z));
   return p;                                                              // the caller sends `near` anchors to project_anchor_f64
 }
 

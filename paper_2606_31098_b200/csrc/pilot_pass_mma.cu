@@ -32,14 +32,10 @@ typedef void (*pass_fn)(const PassArgs);
 template <class T>
 pass_fn pick_mma(int g) {
   switch (g) {
-#ifndef PILOT_FAST_BUILD
     case 2: return photo_pass_kernel<T, 2, false, true>;
-#endif
     case 4: return photo_pass_kernel<T, 4, false, true>;
     case 8: return photo_pass_kernel<T, 8, false, true>;
-#ifndef PILOT_FAST_BUILD
     case 16: return photo_pass_kernel<T, 16, false, true>;
-#endif
   }
   return nullptr;
 }

@@ -200,20 +200,12 @@ typedef void (*resident_fn)(const PassArgs);
 template <class T, bool CEN>
 resident_fn pick_g(int g) {
   switch (g) {
-#ifndef PILOT_FAST_BUILD
     case 1: return lm_resident_kernel<T, 1, CEN, false>;
-#endif
-#ifndef PILOT_FAST_BUILD
     case 2: return lm_resident_kernel<T, 2, CEN, false>;
-#endif
     case 4: return lm_resident_kernel<T, 4, CEN, false>;
     case 8: return lm_resident_kernel<T, 8, CEN, false>;
-#ifndef PILOT_FAST_BUILD
     case 16: return lm_resident_kernel<T, 16, CEN, false>;
-#endif
-#ifndef PILOT_FAST_BUILD
     case 32: return lm_resident_kernel<T, 32, CEN, false>;
-#endif
   }
   return nullptr;
 }
@@ -221,14 +213,10 @@ resident_fn pick_g(int g) {
 template <class T>
 resident_fn pick_mma(int g) {
   switch (g) {
-#ifndef PILOT_FAST_BUILD
     case 2: return lm_resident_kernel<T, 2, false, true>;
-#endif
     case 4: return lm_resident_kernel<T, 4, false, true>;
     case 8: return lm_resident_kernel<T, 8, false, true>;
-#ifndef PILOT_FAST_BUILD
     case 16: return lm_resident_kernel<T, 16, false, true>;
-#endif
   }
   return nullptr;
 }
@@ -236,10 +224,8 @@ resident_fn pick_mma(int g) {
 template <bool CEN>
 resident_fn pick_t(pilot_dtype d, int g) {
   switch (d) {
-#ifndef PILOT_FAST_BUILD      /* tuning builds (-DPILOT_FAST_BUILD): bf16, 32 and 64 channels only */
     case PILOT_F32: return pick_g<F32Tag, CEN>(g);
     case PILOT_F16: return pick_g<F16Tag, CEN>(g);
-#endif
     case PILOT_BF16: return pick_g<BF16Tag, CEN>(g);
   }
   return nullptr;
