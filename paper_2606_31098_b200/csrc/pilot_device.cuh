@@ -774,11 +774,42 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
 
     // ---- rounds
     const int nr = (nv + 7) >> 3;
+    // The ten Gram entries of a row-group's unit from its four difference vectors (one load = KS k-steps), PRODUCT-MAJOR:
+    // the KS k-steps of one product run back to back on one accumulator quad, the two wanted entries of it are kept, and
+    // the next product reuses the quad - 4 + 10 accumulator registers live instead of 6 x 4 (k-step-major order, all six
+    // products side by side: config 4 7.11 ms against 7.01, config 2 6.85 against 6.76 at the same 80 registers). Thread
+    // (g, g / 2) then hands the entries to row `slot` of the warp's buffer.
+    auto contract_and_hand_off = [&](const unsigned (&e0)[NW], const unsigned (&e1)[NW], const unsigned (&e2)[NW], const unsigned (&e3)[NW],
+                                     int slot, bool act) {
+      auto product = [&](const unsigned (&alo)[NW], const unsigned (&ahi)[NW], const unsigned (&b)[NW], float& lo, float& hi) {
+        float c[4];
+        M::mma0(c, alo[0], ahi[0], alo[1], ahi[1], b[0], b[1]);
+#pragma unroll
+        for (int k = 1; k < KS; ++k) M::mma(c, alo[2 * k], ahi[2 * k], alo[2 * k + 1], ahi[2 * k + 1], b[2 * k], b[2 * k + 1]);
+        lo = odd ? c[1] : c[0];                                             // C[g][g]
+        hi = odd ? c[3] : c[2];                                             // C[g + 8][g]
+      };
+      float E00, E02, E01, E12, E03, E23, E22, E11, E13, E33, dup;
+      product(e0, e2, e0, E00, E02);                                        // e0.e0 | e2.e0
+      product(e0, e2, e1, E01, E12);                                        // e0.e1 | e2.e1
+      product(e0, e2, e3, E03, E23);                                        // e0.e3 | e2.e3
+      product(e0, e2, e2, dup, E22);                                        // (e0.e2) | e2.e2
+      product(e1, e3, e1, E11, E13);                                        // e1.e1 | e3.e1
+      product(e1, e3, e3, dup, E33);                                        // (e1.e3) | e3.e3
+      if (diag && act) {
+        const unsigned rp = rows_s + (unsigned)(slot * Geo::kRow) * 4u;
+        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp), "f"(E00), "f"(E01), "f"(E02), "f"(E03) : "memory");
+        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" :: "r"(rp + 16u), "f"(E11), "f"(E12), "f"(E13), "f"(E22) : "memory");
+        asm volatile("st.shared.v2.f32 [%0], {%1,%2};" :: "r"(rp + 32u), "f"(E23), "f"(E33) : "memory");
+      }
+    };
 #if PILOT_MMA_PIPE
     if constexpr (Geo::PARTS == 1) {
       // Software pipeline over the rounds: the next round's five loads are issued as soon as this round's taps have been
       // turned into differences (their registers are free again), so they are in flight during the 6 KS mma.sync and the
       // hand-off of this round - a warp always has loads outstanding, whatever phase the other warps of the SM are in.
+      // (k-step-major order of the products here: at 16 warps per SM the six independent accumulators are worth more than
+      // the registers - product-major measured 0.470 against 0.458 ms on config 1, 0.791 against 0.781 on config 3.)
       TapWords<NW> t[5];
       auto issue = [&](int r) {
         const int s = 8 * r + g;
@@ -839,6 +870,29 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       }
     } else
 #endif
+    if constexpr (Geo::PARTS == 1) {
+      for (int r = 0; r < nr; ++r) {
+        const int s = 8 * r + g;
+        const bool act = s < nv;
+        // a row-group past the last visible unit repeats slot 0 (always there: its loads hit L1) and stores nothing
+        const uint2 sl = slotA[act ? s : 0];
+        const char* const p0 = featq + sl.x;
+        const TapWords<NW> f00 = ldg_words<NW>(p0);
+        const TapWords<NW> f10 = ldg_words<NW>(p0 + PX);
+        const TapWords<NW> f01 = ldg_words<NW>(p0 + row_stride);
+        const TapWords<NW> f11 = ldg_words<NW>(p0 + row_stride + PX);
+        const TapWords<NW> fr = ldg_words<NW>(refq + (size_t)sl.y * PX);
+        unsigned e0[NW], e1[NW], e2[NW], e3[NW];
+#pragma unroll
+        for (int i = 0; i < NW; ++i) {
+          e0[i] = M::sub2(f10.w[i], f00.w[i]);
+          e1[i] = M::sub2(f11.w[i], f01.w[i]);
+          e2[i] = M::sub2(f01.w[i], f00.w[i]);
+          e3[i] = M::sub2(fr.w[i], f01.w[i]);
+        }
+        contract_and_hand_off(e0, e1, e2, e3, s, act);
+      }
+    } else
     for (int r = 0; r < nr; ++r) {
       const int s = 8 * r + g;
       const bool act = s < nv;
