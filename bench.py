@@ -27,7 +27,7 @@ LIGHT = ("poses", "cost", "n_valid", "status", "iter_hessian", "iter_gradient", 
 # captures of this command (profiles/<file>): the first EVAL pass of a timed step (hypotheses spread over their initial
 # poses: the union of their footprints covers the map) and a late pass (hypotheses converged onto one pose). None where
 # no capture of that workload exists. Labelled with their source; everything else in the line is measured in this run.
-NCU_TRAFFIC = {"config4": {"first_pass_bytes": 429.0e6, "converged_pass_bytes": 31.5e6,
+NCU_TRAFFIC = {"config4": {"first_pass_bytes": 420.1e6, "converged_pass_bytes": 31.6e6,
                            "source": "profiles/r2_photo_config4.md"}}
 
 

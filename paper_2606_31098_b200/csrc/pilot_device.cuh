@@ -427,11 +427,6 @@ template <> struct MmaType<F32Tag> {};   // never instantiated: fp32 features st
 #define PILOT_MMA_PROJ_ILP 0       // 1: the projection passes of a super-batch side by side (pass kernel: config 4 -0.8 %;
                                     // the resident kernel, whose levels can be smaller than a super-batch, loses 1-3 %)
 #endif
-#ifndef PILOT_MMA_PROJ_F32
-#define PILOT_MMA_PROJ_F32 1       // 1: projection and visibility of the 16-bit path in fp32 (SURVEY 8(a) a2's number type): the
-                                    // centre as a hi + lo pair of floats, the rotation rounded to float; 16 floats behind the
-                                    // double pose in shared memory
-#endif
 #ifndef PILOT_MMA_SB
 #define PILOT_MMA_SB 64             // anchors a warp projects and compacts before it runs their rounds and lifts them
                                     // (64: 5 KB of shared memory per warp; the resident kernel uses 128)
@@ -586,7 +581,8 @@ __device__ __forceinline__ ProjUnit project_anchor_f32(float Px, float Py, float
 //
 // Same contract as photo_accumulate below (which dispatches here for MMA = true). A warp works on super-batches of SB
 // anchors (SB / 32 of its round-robin batches), in three phases:
-//   project    lane-per-anchor, SB / 32 passes: anchor load, projection + visibility in fp64 (a2). The VISIBLE units are
+//   project    lane-per-anchor, SB / 32 passes: anchor load, projection in fp32 with visibility decided in double near the
+//              borders (a2; project_anchor_f32 / _f64 above). The VISIBLE units are
 //              compacted (ballot + popc rank, running count): slot s of the warp's table gets {tap offset, anchor index} and
 //              the lane-phase state {a, b, X/Z, Y/Z, 1/Z, w_ref}; invisible anchors cost nothing beyond this point;
 //   rounds     ceil(n_visible / 8) rounds; row-group g takes slot 8 r + g: five loads, four packed differences per word,
@@ -610,8 +606,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
   // The candidate pose stays in SHARED memory (Rc[9] and Ccand = Rc + 9 must point there, 16-byte aligned) and is re-read
   // by every projection: as 24 registers held across the rounds it forced the address arithmetic to be rematerialised.
   const unsigned pose_s = (unsigned)__cvta_generic_to_shared(Rc);         // Rc[9] | Cc[3] contiguous, 16-byte aligned
-  const double wmax = (double)(L.W - 1), hmax = (double)(L.H - 1);
-  (void)wmax; (void)hmax;
   const float wmaxf = (float)(L.W - 1), hmaxf = (float)(L.H - 1);
   const float band = 4e-6f * (fabsf(L.fx) + fabsf(L.fy) + (float)(L.W + L.H));   // see project_anchor_f32
 
@@ -638,7 +632,7 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
     // ---- project + compact
     int nv = 0;
 #if PILOT_MMA_PROJ_ILP
-    // the SB / 32 passes are independent fp64 chains: written out side by side so that the compiler interleaves them (a
+    // the SB / 32 passes are independent chains: written out side by side so that the compiler interleaves them (a
     // batch past the end projects nothing: its lanes are invalid). The first pass's anchors were loaded one super-batch ago.
     {
       float4 Pk[PASSES];
@@ -649,7 +643,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       float pa[PASSES], pb[PASSES], px[PASSES], py[PASSES], piz[PASSES];
       unsigned poff[PASSES];
       bool pvalid[PASSES];
-#if PILOT_MMA_PROJ_F32
       bool pnear[PASSES];
       float Rf[16];                                                       // R[9], C hi[3], C lo[3], pad: four 16-byte loads
 #pragma unroll
@@ -675,33 +668,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
           pa[k] = pu.a; pb[k] = pu.b; px[k] = pu.x; py[k] = pu.y; piz[k] = pu.iz; poff[k] = pu.off; pvalid[k] = pu.valid;
         }
       }
-#else
-      double R[12];                                                       // six 16-byte shared-memory loads
-#pragma unroll
-      for (int i = 0; i < 6; ++i)
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
-      const double* Cc = R + 9;
-#pragma unroll
-      for (int k = 0; k < PASSES; ++k) {
-        const int base = begin + (b0 + k * n_workers) * 32;
-        bool valid = (b0 + k * n_workers) < n_batches && base + lane < end;
-        double dx = (double)Pk[k].x - Cc[0], dy = (double)Pk[k].y - Cc[1], dz = (double)Pk[k].z - Cc[2];
-        double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
-        double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
-        double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
-        valid = valid && (Zd > (double)A.prm.z_near);
-        double izd = fast_rcp(Zd);
-        double ud = (double)L.fx * Xd * izd + (double)L.cx;
-        double vd = (double)L.fy * Yd * izd + (double)L.cy;
-        double x0d = floor(ud), y0d = floor(vd);
-        valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
-        const float iz = (float)izd;
-        pa[k] = (float)(ud - x0d); pb[k] = (float)(vd - y0d);
-        px[k] = (float)Xd * iz; py[k] = (float)Yd * iz; piz[k] = iz;
-        poff[k] = valid ? ((unsigned)(int)y0d * (unsigned)L.W + (unsigned)(int)x0d) * (unsigned)PX : 0u;
-        pvalid[k] = valid;
-      }
-#endif
 #pragma unroll
       for (int k = 0; k < PASSES; ++k) {
         const unsigned vmask = __ballot_sync(0xffffffffu, pvalid[k]);
@@ -724,7 +690,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
       const float4 P = Pn;
       Pn = load_anchor(b + n_workers);                                    // next pass's anchors: in flight during this one
       bool valid = base + lane < end;
-#if PILOT_MMA_PROJ_F32
       float Rf[16];                                                       // R[9], C hi[3], C lo[3], pad: four 16-byte loads
 #pragma unroll
       for (int i = 0; i < 4; ++i)
@@ -740,32 +705,6 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
         slotB[s] = make_float4(pu.a, pu.b, pu.x, pu.y);
         slotC[s] = make_float2(pu.iz, P.w);
       }
-#else
-      double R[12];                                                       // six 16-byte shared-memory loads
-#pragma unroll
-      for (int i = 0; i < 6; ++i)
-        asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(R[2 * i]), "=d"(R[2 * i + 1]) : "r"(pose_s + 16u * i));
-      const double* Cc = R + 9;
-      double dx = (double)P.x - Cc[0], dy = (double)P.y - Cc[1], dz = (double)P.z - Cc[2];
-      double Xd = R[0] * dx + R[1] * dy + R[2] * dz;
-      double Yd = R[3] * dx + R[4] * dy + R[5] * dz;
-      double Zd = R[6] * dx + R[7] * dy + R[8] * dz;
-      valid = valid && (Zd > (double)A.prm.z_near);
-      double izd = fast_rcp(Zd);
-      double ud = (double)L.fx * Xd * izd + (double)L.cx;
-      double vd = (double)L.fy * Yd * izd + (double)L.cy;
-      double x0d = floor(ud), y0d = floor(vd);
-      valid = valid && (x0d >= 0.0) && (y0d >= 0.0) && (x0d + 1.0 <= wmax) && (y0d + 1.0 <= hmax);
-      const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-      if (valid) {
-        const int s = nv + __popc(vmask & ((1u << lane) - 1u));
-        const unsigned off = ((unsigned)(int)y0d * (unsigned)L.W + (unsigned)(int)x0d) * (unsigned)PX;
-        const float iz = (float)izd;
-        slotA[s] = make_uint2(off, (unsigned)(base + lane));
-        slotB[s] = make_float4((float)(ud - x0d), (float)(vd - y0d), (float)Xd * iz, (float)Yd * iz);
-        slotC[s] = make_float2(iz, P.w);
-      }
-#endif
       nv += __popc(vmask);
     }
 #endif
@@ -774,11 +713,12 @@ __device__ __forceinline__ void photo_accumulate_mma(const PassArgs& A, const do
 
     // ---- rounds
     const int nr = (nv + 7) >> 3;
-    // The ten Gram entries of a row-group's unit from its four difference vectors (one load = KS k-steps), PRODUCT-MAJOR:
-    // the KS k-steps of one product run back to back on one accumulator quad, the two wanted entries of it are kept, and
-    // the next product reuses the quad - 4 + 10 accumulator registers live instead of 6 x 4 (k-step-major order, all six
-    // products side by side: config 4 7.11 ms against 7.01, config 2 6.85 against 6.76 at the same 80 registers). Thread
-    // (g, g / 2) then hands the entries to row `slot` of the warp's buffer.
+    // The ten Gram entries of a row-group's unit from its four difference vectors (one load = KS k-steps), written
+    // PRODUCT-MAJOR: the KS k-steps of one product on one accumulator quad, its two wanted entries kept, then the next
+    // product. ptxas still interleaves the six quads (the SASS keeps 24 accumulator registers), but from this order it
+    // needs fewer register-pairing copies around the HMMAs than from the k-step-major one (132 instead of 146 instructions
+    // per round): config 4 7.11 -> 7.00 ms, config 2 6.85 -> 6.76 at the same 80 registers. Thread (g, g / 2) then hands
+    // the entries to row `slot` of the warp's buffer.
     auto contract_and_hand_off = [&](const unsigned (&e0)[NW], const unsigned (&e1)[NW], const unsigned (&e2)[NW], const unsigned (&e3)[NW],
                                      int slot, bool act) {
       auto product = [&](const unsigned (&alo)[NW], const unsigned (&ahi)[NW], const unsigned (&b)[NW], float& lo, float& hi) {

@@ -21,9 +21,7 @@ __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(
     if constexpr (MMA) {                          // the tensor-core gather re-reads the pose from shared memory
       __shared__ __align__(16) double s_pose[12 + 8];       // Rc[9] | Cc[3] | 16 floats: R, centre hi, centre lo (fp32 projection)
       if (threadIdx.x < 12) s_pose[threadIdx.x] = threadIdx.x < 9 ? st->Rc[threadIdx.x] : st->Cc[threadIdx.x - 9];
-#if PILOT_MMA_PROJ_F32
       else if (threadIdx.x < 32 + 16 && threadIdx.x >= 32) pose_to_float(st->Rc, st->Cc, (int)threadIdx.x - 32, reinterpret_cast<float*>(s_pose + 12));
-#endif
       __syncthreads();
       Rc = s_pose; Cc = s_pose + 9;
     }
