@@ -21,7 +21,7 @@ def with_hypotheses(prob, n, seed=5):
     return p
 
 
-def gpu_and_oracle(prob, params, mode="auto", weights=None, teacher=False):
+def gpu_and_oracle(prob, params, mode="auto", weights=None, teacher=False, sup_level=0):
     """GPU forward with the extra records + GPU chain, oracle forward + oracle chain. teacher=True: the GPU chain reads the
     ORACLE's records (rounded to fp32 and uploaded) instead of its own forward's, so that both chains differentiate the very
     same trajectory - for inputs whose free-running trajectories drift apart (rough maps, bf16 features)."""
@@ -37,8 +37,9 @@ def gpu_and_oracle(prob, params, mode="auto", weights=None, teacher=False):
     out = r.run(di, params)
     torch.cuda.synchronize()
     out_np = {k: v.cpu().numpy().copy() for k, v in out.items()}
-    pts = torch.from_numpy(np.ascontiguousarray(prob["points"][0], np.float32)).to(d)
-    K = prob["intrinsics"][0]
+    sl = sup_level                          # the level whose camera and anchors define the reprojection supervision
+    pts = torch.from_numpy(np.ascontiguousarray(prob["points"][sl], np.float32)).to(d)
+    K = prob["intrinsics"][sl]
     Tstar = np.asarray(prob["gt_pose"], np.float32)
     orc = po.run(po.Bound(prob, params))
     T, H = orc["iter_poses"].shape[:2]
@@ -50,22 +51,29 @@ def gpu_and_oracle(prob, params, mode="auto", weights=None, teacher=False):
         rec = dict(iter_hessian=up(orc["iter_hessian"], np.float32), iter_gradient=up(orc["iter_gradient"], np.float32),
                    iter_lambda=up(orc["iter_lambda"], np.float32), iter_poses=up(orc["iter_poses"], np.float32),
                    iter_accept=up(acc, np.int32), poses=up(orc["poses64"], np.float32))
-    g = binding.unrolled_backward(r, di, params, rec, Tstar, pts, K, prob["width"][0], prob["height"][0], ALPHA, SCALE,
+    g = binding.unrolled_backward(r, di, params, rec, Tstar, pts, K, prob["width"][sl], prob["height"][sl], ALPHA, SCALE,
                                   step_weights=weights, grad_conf=True)
     torch.cuda.synchronize()
     K32 = [float(np.float32(k)) for k in K]
-    og = pu.unrolled_backward(prob, params, orc, Tstar, prob["points"][0], K32, prob["width"][0], prob["height"][0], ALPHA, SCALE,
+    og = pu.unrolled_backward(prob, params, orc, Tstar, prob["points"][sl], K32, prob["width"][sl], prob["height"][sl], ALPHA, SCALE,
                               step_weights=weights)
     r.close()
-    return dict(out=out_np, g=g, orc=orc, og=og, acc=acc)
+    return dict(out=out_np, g=g, orc=orc, og=og, acc=acc, first_level_solves=int(params["iters"][0]))
 
 
-def check(res, n_levels, tol, pose_tol=1e-3):
-    """pose_tol: the free-running iterates against the oracle's (north_star: 1e-3 for fp32 features, 5e-3 for bf16)."""
+def check(res, n_levels, tol, pose_tol=1e-3, strict_accept=True):
+    """pose_tol: the free-running iterates against the oracle's (north_star: 1e-3 for fp32 features, 5e-3 for bf16).
+    strict_accept=False: near convergence the cost differences that decide accept / reject are at the level of the bf16
+    rounding, so the free-running GPU run may reject a late step the oracle accepts (reading A19: compare what is unique) -
+    the flags must then agree on every solve of the first level and on at least 80 % of all solves."""
     out, g, og = res["out"], res["g"], res["og"]
     # the extra records of the forward run: iterate poses and accept flags
     assert np.abs(out["iter_poses"] - res["orc"]["iter_poses"]).max() <= pose_tol
-    assert np.array_equal(out["iter_accept"].astype(bool), res["acc"])
+    if strict_accept:
+        assert np.array_equal(out["iter_accept"].astype(bool), res["acc"])
+    else:
+        same = out["iter_accept"].astype(bool) == res["acc"]
+        assert same[:res["first_level_solves"]].all() and same.mean() >= 0.8, same
     assert np.allclose(g["loss"].cpu().numpy(), og["loss"], rtol=tol, atol=1e-6)
     gi = g["grad_init_pose"].cpu().numpy()
     assert np.abs(gi - og["grad_init_pose"]).max() <= tol * np.abs(og["grad_init_pose"]).max()
@@ -101,6 +109,23 @@ def test_confidence_maps_weights_and_bf16():
     params = dict(iters=[2, 2], loss="huber", loss_scale=0.5, lm_mode="adaptive", lambda_init=1.0, min_valid=4, w_gravity=0.0,
                   range_mode="off", z_near=ZN)
     check(gpu_and_oracle(p, params, "auto", weights=[0.1, 0.2, 0.3, 0.4], teacher=True), 2, 2e-3, pose_tol=5e-3)
+
+
+def test_paper_shape_nine_unrolled_steps():
+    """The paper's own training shape (supp III-B/C): 500 geo-anchors, a three-level pyramid of L2-normalised
+    32-channel descriptors with query and reference confidences, 2 + 3 + 4 = nine unrolled steps, the objective the average
+    of the nine per-step reprojection losses in the full-resolution camera. Synthetic stand-in for its data
+    (workloads.paper_frame); priors off (the chain differentiates the photo term)."""
+    from paper_2606_31098_b200 import workloads as wl
+    prob = wl.paper_frame(N=500, iters=(2, 3, 4), dtype="bf16")
+    params = dict(prob["params"], w_gravity=0.0, range_mode="off")
+    rng = np.random.default_rng(17)
+    prob["init_poses"] = np.stack([_perturb(prob["gt_pose"], np.concatenate([rng.uniform(-3, 3, 3), rng.uniform(-0.02, 0.02, 3)]))
+                                   for _ in range(2)]).astype(np.float32)
+    res = gpu_and_oracle(prob, params, "auto", teacher=True, sup_level=2)
+    assert res["out"]["iter_accept"].shape == (9, 2) and res["out"]["iter_accept"].sum() >= 12
+    check(res, 3, 2e-3, pose_tol=5e-3, strict_accept=False)
+    assert float(res["g"]["loss"].min()) > 0.0
 
 
 def test_rejected_steps():
