@@ -1,6 +1,6 @@
 // pilot_pass.cuh — the one-launch-per-pass photo kernel, shared by the two translation units
 // that instantiate it with different CTA shapes: pilot_refine.cu (FFMA2 contraction: 4 warps, 128 registers) and
-// pilot_pass_mma.cu (tensor-core contraction: 4 warps, 72 registers, 28 warps per SM). Shares no code with oracle/.
+// pilot_pass_mma.cu (tensor-core contraction: 4 warps, 80 registers, 24 warps per SM). Shares no code with oracle/.
 #pragma once
 #include "pilot_device.cuh"
 

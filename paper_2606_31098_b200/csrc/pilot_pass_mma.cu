@@ -6,7 +6,9 @@
 // (B200, ms per step): 16 warps at 128 registers 8.76 (8.31 with the next round's taps prefetched), 20 warps at 96: 8.17,
 // 24 at 80: 7.88, 28 at 72: 7.94, 32 at 64: 8.30; CTAs of 2 / 8 warps at the same occupancy 7.94 / 8.02; anchors per CTA
 // 768 ... 3072: 7.83-7.87 (1536 kept). Round 1's layout (a unit split over two row-groups, 28 warps at 72 registers): 7.65
-// with the empty batches skipped, 8.98 without. Shares no code with oracle/.
+// with the empty batches skipped, 8.98 without. Later changes of round 2 (staged finalisation, fp32 projection, product-major
+// Gram order: pilot_device.cuh) took the 7.88 of this sweep to 7.00 at the same shape; re-checked then: 72 / 64 registers
+// 7.51 / 8.76, super-batch 64 / 128: 7.14 / 7.73, anchors per CTA 1024 ... 2304: 7.03-7.25. Shares no code with oracle/.
 #ifndef PILOT_MMA_THREADS
 #define PILOT_MMA_THREADS 128
 #define PILOT_MMA_MIN_BLOCKS 6
