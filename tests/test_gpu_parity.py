@@ -197,6 +197,24 @@ def test_visibility_is_decided_in_double(shift):
             check_systems(gpu, orc, "bf16", recs=(0, 1, 2))
 
 
+@pytest.mark.parametrize("shift", [(0.0, 0.0, 0.0), (5000.0, -3200.0, 150.0)])
+def test_fp32_projection_far_from_the_local_origin(shift):
+    """The tensor-core path projects in fp32 with the camera centre as a hi + lo pair of floats: a scene 6 km from the origin
+    of the world frame (anchors quantised to 0.5 mm by their own fp32 storage, identically on both sides) must give the same
+    systems as the oracle's double projection, and the same visible set - at the input poses and, teacher-forced, at the
+    oracle's own iterates."""
+    prob = tiny(seed=43, N=900, C=32, n_hyp=4, dtype="bf16", conf=True, W=64, H=48, origin_shift=shift)
+    P = dict(iters=[3], loss="huber", loss_scale=0.4, min_valid=4)
+    gpu, orc = both(prob, P)
+    check_systems(gpu, orc, "bf16", recs=(0,))
+    assert np.array_equal(gpu["n_valid"], orc["n_valid"])
+    for rec in (1, 2):
+        tf = parity.level_slice(dict(prob, params=P), 0, orc["iter_poses"][rec], iters=1)
+        g2, o2 = both(tf)
+        check_systems(g2, o2, "bf16", recs=(0,))
+        assert np.array_equal(g2["n_valid"], o2["n_valid"])
+
+
 def test_run_is_deterministic():
     from paper_2606_31098_b200 import binding
     prob = wl.config1(H=16, N=1500, iters=(3, 3, 3))
