@@ -484,6 +484,40 @@ def measure(W, steps, warmup, stream, local_rank, world, use_dist, flush):
             "clocks": sampler.summary(), "visible_evals": vis, "all_evals": tot}
 
 
+def measure_graph(W, steps, local_rank, flush):
+    """The same step captured once into a CUDA graph and replayed (what a serving loop does with a launch-bound step: the
+    library's calls are capturable - no allocation, no host synchronisation). Returns ms per step, or None if the capture
+    fails. Timed like measure(): CUDA events around every replay, the L2 flush outside them."""
+    import torch
+    try:
+        side = torch.cuda.Stream(device=local_rank)
+        side.wait_stream(torch.cuda.current_stream(local_rank))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            W.step(side)                                   # allocations of the binding settle before the capture
+            side.synchronize()
+            with torch.cuda.graph(g, stream=side):
+                W.step(side)
+        torch.cuda.synchronize(local_rank)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize(local_rank)
+        cur = torch.cuda.current_stream(local_rank)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for s, e in ev:
+            if flush is not None:
+                flush.fill_(1)
+            s.record(cur)
+            g.replay()
+            e.record(cur)
+        torch.cuda.synchronize(local_rank)
+        W.check()
+        return sum(s.elapsed_time(e) for s, e in ev) / steps
+    except Exception as ex:                                # noqa: BLE001  (reported, not fatal: the stream-launched figure stands)
+        sys.stderr.write(f"[bench] CUDA-graph leg skipped: {ex}\n")
+        return None
+
+
 def roofline_of(W, m, name, peaks, hbm_peak, hbm_src, map_bytes, l2_bytes):
     """The dominant kernel's roofline. What binds is the gather of the taps from L2 into the SMs (the
     maps are L2-resident, or - config 4 - the union of the co-resident CTAs' footprints is: 30-420 MB of DRAM traffic per
@@ -575,6 +609,7 @@ def run_workload(name, args, rank, local_rank, world, use_dist, stream, steps, p
     warmup = max(3, args.warmup)
     m = measure(W, steps, warmup, stream, local_rank, world, use_dist, flush)
     roof = roofline_of(W, m, name, peaks, hbm[0], hbm[1], map_bytes, l2_bytes)
+    graph_ms = measure_graph(W, steps, local_rank, flush) if (name in ("config1", "paper") and world == 1) else None
     e2e = None
     if with_e2e:
         n_e2e = max(1, min(steps, 10))
@@ -605,6 +640,9 @@ def run_workload(name, args, rank, local_rank, world, use_dist, stream, steps, p
     res = {"ms_per_step": m["ms_per_step"], "value": m["value"], "steps": steps, "warmup": warmup, "dtype": dtype_string(W),
            "config": cfg, "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(m["launches"] * steps),
            "clocks": m["clocks"]}
+    if graph_ms is not None:
+        res["cuda_graph"] = {"ms_per_step": graph_ms, "value": W.units / (graph_ms * 1e-3), "unit": UNIT,
+                             "note": "the same step captured once and replayed (launch gaps removed); ms_per_step above is stream-launched"}
     W.close()
     del W, flush
     torch.cuda.empty_cache()
@@ -671,6 +709,8 @@ def main():
             others[name]["roofline"] = {k: r["roofline"].get(k) for k in ("bound", "achieved", "peak", "unit", "frac", "kernel",
                                                                           "visible_fraction", "contraction", "pass_ms")}
             others[name]["roofline"]["hbm_no_reuse_frac_all_units"] = r["roofline"]["hbm_no_reuse"]["frac_all_units"]
+            if "cuda_graph" in r:
+                others[name]["cuda_graph"] = r["cuda_graph"]
 
     if rank == 0:
         cfg = main_res["config"]
@@ -684,6 +724,8 @@ def main():
                 "scaling": "weak", "vs_baseline": None, "dtype": main_res["dtype"], "data": "synthetic", "config": cfg,
                 "roofline": main_res["roofline"], "cpu_baseline": main_res["cpu_baseline"], "e2e": main_res["e2e"],
                 "gpu_launches": main_res["gpu_launches"], "clocks": main_res["clocks"]}
+        if "cuda_graph" in main_res:
+            line["cuda_graph"] = main_res["cuda_graph"]
         if others is not None:
             line["other_workloads"] = others
         print(json.dumps(line))
