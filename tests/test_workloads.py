@@ -28,6 +28,7 @@ def test_paper_counts_arithmetic():
     assert p["channels"] == [g["descriptor_channels"]] * 3 and p["points"][0].shape[0] == g["geo_anchors"]
     assert p["params"]["iters"] == [g["iters_coarse"], g["iters_medium"], g["iters_fine"]]
     assert len(wl.PAPER_YAWS) == 10 and 0.0 not in wl.PAPER_YAWS
+    assert g["unrolled_training_steps"] == g["iters_coarse"] + g["iters_medium"] + g["iters_fine"]   # PAPER.md:440 and :205 agree
 
 
 def test_paper_frame_is_normalised_and_weighted():
