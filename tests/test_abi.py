@@ -77,3 +77,42 @@ def test_oracle_types_describe_the_same_bytes_as_the_abi_header():
     for name, text in orc.items():
         assert abi.get(name) == text, name
     assert "pilot_refine.h" not in re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "oracle", "pilot_oracle.h")).read(), flags=re.S)
+
+
+def test_unrolled_backward_argument_checks_need_no_gpu():
+    """pilot_refine_unrolled_backward refuses bad arguments before any CUDA call: NULL structs, priors on (their
+    pose-dependence is not part of the chain), the sampled-gradient mode, missing records, a scratch buffer that is too small."""
+    from paper_2606_31098_b200 import binding
+    L = binding.lib()
+    sb = L.pilot_refine_unrolled_backward_scratch_bytes
+    assert sb(-1, 3) == 0 and sb(4, -1) == 0 and sb(0, 0) % 256 == 0
+    assert 0 < sb(2, 3) <= sb(4, 3) <= sb(4, 9) and sb(4, 9) % 256 == 0
+    cfg = binding.Config()
+    cfg.n_levels, cfg.feat_dtype = 2, 1
+    for l in range(2):
+        cfg.width[l], cfg.height[l], cfg.channels[l] = 64, 48, 32
+    inp = binding.Inputs()
+    inp.n_hypotheses = 2
+    par, _ = binding.make_params(dict(iters=[1, 2], w_gravity=0.0, range_mode="off"), 2)
+    rec, sup, g = binding.UnrolledRecords(), binding.Supervision(), binding.UnrolledGrads()
+    call = lambda c, i, p, r, s_, o, scratch=None, nbytes=0: L.pilot_refine_unrolled_backward(
+        ctypes.byref(c) if c else None, ctypes.byref(i) if i else None, ctypes.byref(p) if p else None,
+        ctypes.byref(r) if r else None, ctypes.byref(s_) if s_ else None, ctypes.byref(o) if o else None, scratch, nbytes, None)
+    assert call(None, inp, par, rec, sup, g) == -1
+    assert call(cfg, inp, par, None, sup, g) == -1
+    assert call(cfg, inp, par, rec, sup, g) == -1                          # records and supervision points missing
+    pg, _ = binding.make_params(dict(iters=[1, 2], w_gravity=1.0, range_mode="off"), 2)
+    assert call(cfg, inp, pg, rec, sup, g) == -3
+    pr, _ = binding.make_params(dict(iters=[1, 2], w_gravity=0.0, range_mode="march", w_range=1.0), 2)
+    assert call(cfg, inp, pr, rec, sup, g) == -3
+    pc, _ = binding.make_params(dict(iters=[1, 2], w_gravity=0.0, range_mode="off", grad_mode="central_sampled"), 2)
+    assert call(cfg, inp, pc, rec, sup, g) == -3
+    # everything present (fake non-NULL addresses, never dereferenced on this path) but no scratch: PILOT_ERR_WORKSPACE
+    w = (ctypes.c_float * 3)(1 / 3, 1 / 3, 1 / 3)
+    for f in ("iter_hessian_dev", "iter_gradient_dev", "iter_lambda_dev", "iter_poses_dev", "iter_accept_dev", "final_poses_dev"):
+        setattr(rec, f, 256)
+    sup.points_dev, sup.n_points, sup.step_weights = 256, 1, ctypes.cast(w, ctypes.POINTER(ctypes.c_float))
+    assert call(cfg, inp, par, rec, sup, g) == -2
+    assert call(cfg, inp, par, rec, sup, g, 256, 16) == -2
+    inp.n_hypotheses = 0
+    assert call(cfg, inp, par, rec, sup, g) == 0                           # nothing to do
