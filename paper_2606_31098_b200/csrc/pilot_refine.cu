@@ -449,12 +449,12 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
         return PILOT_ERR_CUDA;
       }
       dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
-      // small CTAs (<= 512 anchors) in more than one wave, or many hypotheses (measured: config 2, H = 1024, -4 %):
-      // the serial tail moves to its own launch
+      // small CTAs (<= 512 anchors) in more than one wave, or many hypotheses (measured: config 2, H = 1024, 7.01 -> 6.76 ms;
+      // config 4, H = 256, 7.01 -> 6.97): the serial tail moves to its own launch
       const int per_cta = A.chunk < L.N ? A.chunk : L.N;
       A.defer = h->mode == PILOT_EXEC_PASSES_SPLIT ||
                 (h->mode == PILOT_EXEC_AUTO &&
-                 ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 512));
+                 ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 256));
       for (int pass = 0; pass <= p->iters[l]; ++pass) {
         A.pass = pass;
         if (mma) {
