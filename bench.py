@@ -39,27 +39,39 @@ def load_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML during the timed region."""
+    """Samples SM clock and throttle reasons through NVML during the timed region. NVML is initialised in the constructor
+    (before the region) and the thread samples every 5 ms from its first instruction on, so that even a timed region of a
+    few milliseconds holds samples taken under load."""
 
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
-
-    def run(self):
+        self.nv = self.h = None
         try:
             import pynvml as nv
             nv.nvmlInit()
-            h = nv.nvmlDeviceGetHandleByIndex(self.index)
-            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
-            names = {getattr(nv, n): n for n in dir(nv) if n.startswith("nvmlClocksThrottleReason") and
-                     isinstance(getattr(nv, n), int)}
+            self.nv, self.h = nv, nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+            self.names = {getattr(nv, n): n for n in dir(nv) if n.startswith("nvmlClocksThrottleReason") and
+                          isinstance(getattr(nv, n), int)}
+        except Exception as e:  # pragma: no cover
+            self.reasons.add(f"nvml_error:{type(e).__name__}")
+
+    def sample(self):
+        nv, h = self.nv, self.h
+        self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+        r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+        for bit, n in self.names.items():
+            if bit and (r & bit) == bit and "All" not in n and "None" not in n:
+                self.reasons.add(n.replace("nvmlClocksThrottleReason", ""))
+
+    def run(self):
+        if self.nv is None:
+            return
+        try:
             while not self.stop_flag:
-                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
-                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
-                for bit, n in names.items():
-                    if bit and (r & bit) == bit and "All" not in n and "None" not in n:
-                        self.reasons.add(n.replace("nvmlClocksThrottleReason", ""))
-                time.sleep(0.05)
+                self.sample()
+                time.sleep(0.005)
         except Exception as e:  # pragma: no cover
             self.reasons.add(f"nvml_error:{type(e).__name__}")
 
