@@ -99,6 +99,9 @@ __global__ void __launch_bounds__(kSelThreads) topk_kernel(const float* __restri
   extern __shared__ unsigned long long s[];
   for (int i = threadIdx.x; i < n_pow2; i += kSelThreads) s[i] = i < n ? make_key(cost[i], i) : ~0ull;
   __syncthreads();
+  // A compare-exchange pass with stride <= 32 touches, per warp and per turn of the t loop, only that warp's own block of 64
+  // keys (lo = 2t - (t & (stride-1)) over 32 consecutive t), so those passes - 51 of the 66 of a 2048-key sort - need only a
+  // warp-level barrier; the CTA-wide one separates them from the passes with longer strides.
   for (int size = 2; size <= n_pow2; size <<= 1) {
     for (int stride = size >> 1; stride > 0; stride >>= 1) {
       for (int t = threadIdx.x; t < (n_pow2 >> 1); t += kSelThreads) {
@@ -108,7 +111,7 @@ __global__ void __launch_bounds__(kSelThreads) topk_kernel(const float* __restri
         unsigned long long a = s[lo], b = s[hi];
         if ((a > b) == up) { s[lo] = b; s[hi] = a; }
       }
-      __syncthreads();
+      if (stride > 32 || stride == 1) __syncthreads(); else __syncwarp();
     }
   }
   for (int i = threadIdx.x; i < k; i += kSelThreads) {
