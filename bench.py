@@ -621,7 +621,7 @@ def run_workload(name, args, rank, local_rank, world, use_dist, stream, steps, p
     warmup = max(3, args.warmup)
     m = measure(W, steps, warmup, stream, local_rank, world, use_dist, flush)
     roof = roofline_of(W, m, name, peaks, hbm[0], hbm[1], map_bytes, l2_bytes)
-    graph_ms = measure_graph(W, steps, local_rank, flush) if (name in ("config1", "paper") and world == 1) else None
+    graph_ms = measure_graph(W, steps, local_rank, flush) if (name != "config3" and world == 1) else None
     e2e = None
     if with_e2e:
         n_e2e = max(1, min(steps, 10))
