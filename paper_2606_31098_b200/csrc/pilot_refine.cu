@@ -18,10 +18,19 @@
 #endif
 #include "pilot_pass.cuh"
 
+#include <nvtx3/nvToolsExt.h>   // header-only NVTX 3: ranges show up in nsys / ncu timelines, no-ops when no tool is attached
 #include <stdio.h>
 #include <string.h>
 
 #include <mutex>
+
+namespace {
+// RAII NVTX range (tracing). One per host entry point of the hot path and per pyramid level.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 namespace {
 
@@ -362,6 +371,7 @@ int pilot_refine_run(pilot_refine_handle* h, const pilot_refine_inputs* in, cons
 int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
                             const pilot_refine_outputs* out, int level_begin, int level_end, void* cuda_stream) {
   if (!h || !in || !p || !out) return PILOT_ERR_ARG;
+  NvtxRange nvtx_run("pilot_refine_run_levels");
   const pilot_refine_config& c = h->cfg;
   if (level_begin < 0 || level_begin >= level_end || level_end > c.n_levels) return PILOT_ERR_ARG;
   if (in->n_hypotheses < 0) return PILOT_ERR_ARG;
@@ -419,6 +429,8 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
   int rec_base = 0;
   for (int l = 0; l < level_end; ++l) {
     if (l < level_begin) { rec_base += p->iters[l]; continue; }
+    static const char* const kLevelNames[PILOT_MAX_LEVELS] = {"pilot level 0", "pilot level 1", "pilot level 2", "pilot level 3"};
+    NvtxRange nvtx_level(kLevelNames[l]);
     LevelArgs& L = A.lv;
     L.feat = in->query_feat_dev[l]; L.conf = in->query_conf_dev[l];
     L.points = reinterpret_cast<const float4*>(in->points_dev[l]); L.ref = in->ref_feat_dev[l];
@@ -621,6 +633,7 @@ extern "C" {
 int pilot_refine_submit_host(pilot_refine_handle* h, const pilot_refine_inputs* in, const pilot_refine_params* p,
                              const pilot_refine_outputs* out, void* cuda_stream) {
   if (!h || !in || !p || !out || !h->host_mode) return PILOT_ERR_ARG;
+  NvtxRange nvtx_submit("pilot_refine_submit_host");
   const pilot_refine_config& c = h->cfg;
   int prev = 0;
   cudaGetDevice(&prev);
@@ -688,6 +701,7 @@ int pilot_refine_submit_pruned_host(pilot_refine_handle* h, const pilot_refine_i
                                     const float* prior_pose_host, int keep, int seed_frame, float* best_pose_host,
                                     float* best_cost_host, int* best_index_host, void* cuda_stream) {
   if (!h || !in || !p || !prior_pose_host || !h->host_mode || !h->grid) return PILOT_ERR_ARG;
+  NvtxRange nvtx_submit("pilot_refine_submit_pruned_host");
   const pilot_refine_config& c = h->cfg;
   const int n = h->grid_n;
   if (keep < 1 || keep > n || c.n_levels < 2) return PILOT_ERR_ARG;
@@ -754,6 +768,7 @@ int pilot_refine_submit_pruned_host(pilot_refine_handle* h, const pilot_refine_i
 
 int pilot_refine_wait_host(pilot_refine_handle* h) {
   if (!h || !h->host_mode || h->n_waited >= h->n_submitted) return PILOT_ERR_ARG;
+  NvtxRange nvtx_wait("pilot_refine_wait_host");
   const int half = (int)(h->n_waited & 1);
   h->n_waited += 1;
   return cudaEventSynchronize(h->ev_done[half]) == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
