@@ -83,6 +83,9 @@ struct PassArgs {
   int n_hyp, level, level_end, pass, iters, rec_base;
   int chunk, n_chunks;
   int defer;                // 1: the pass kernel only writes partial sums; finalize_kernel ends the iteration
+  int prior_cta;            // 1 (only with defer): row 0 of the grid's y axis is one CTA per hypothesis that evaluates the priors'
+                            // terms at the candidate pose WHILE the other rows gather; finalize_kernel adds them (struct PriorTerms)
+  void* priors;             // [n_hyp] PriorTerms in the workspace
   // what the finalisation reads as doubles, converted once on the host (an F2F costs the single finalising lane ~18 cycles)
   struct { double lambda_init, lambda_up, lambda_down, lambda_min, lambda_max, w_gravity, gravity_scale, w_range, range_scale,
                   gw[3], gi[3]; } pd;
@@ -1658,12 +1661,13 @@ __device__ void finalize_hypothesis(const PassArgs& A, HypState& s, int m, const
 // The same on the state in the workspace (global memory): the warp stages it through `scratch` (SHARED memory, one
 // HypState per calling warp) with coalesced copies, so that lane 0 works on shared memory instead of chasing 456 bytes
 // of global memory through dependent loads (config 4 7.75 -> 7.57 ms, config 2 7.41 -> 7.33). Warp-collective.
-__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const double* sums, int lane, HypState* scratch) {
+__device__ __noinline__ void finalize_in_workspace(const PassArgs& A, int m, const double* sums, int lane, HypState* scratch,
+                                                   const PriorTerms* pre = nullptr) {
   const int* src = reinterpret_cast<const int*>(A.state + m);
   int* dst = reinterpret_cast<int*>(scratch);
   for (int i = lane; i < (int)(sizeof(HypState) / 4); i += 32) dst[i] = src[i];
   __syncwarp();
-  finalize_hypothesis(A, *scratch, m, sums, lane, nullptr);
+  finalize_hypothesis(A, *scratch, m, sums, lane, pre);
   __syncwarp();
   int* out = reinterpret_cast<int*>(A.state + m);
   for (int i = lane; i < (int)(sizeof(HypState) / 4); i += 32) out[i] = dst[i];

@@ -8,9 +8,20 @@ namespace {
 
 template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
-  const int m = blockIdx.x, chunk_idx = blockIdx.y;
+  const int m = blockIdx.x;
+  int chunk_idx = blockIdx.y;
   const HypState* st = A.state + m;
   if (st->level != A.level) return;             // finished this level early (failed factorisations)
+  if (A.prior_cta) {
+    // Row 0 of the grid: the priors' terms (heightfield ray-march of the range prior, algebra of both: supp Eq.5-6) depend only
+    // on the candidate pose, so one warp per hypothesis evaluates them WHILE the other rows gather, and the deferred
+    // finalisation adds 28 numbers instead of running the march's chain of dependent DSM samples on its own critical path.
+    if (chunk_idx == 0) {
+      if (threadIdx.x < 32) prior_terms_store(A, st->Rc, st->Cc, (int)threadIdx.x, static_cast<PriorTerms*>(A.priors) + m);
+      return;
+    }
+    chunk_idx -= 1;
+  }
 
   PILOT_DECLARE_ACC
   acc_zero<MMA>(acc, sacc);

@@ -45,13 +45,19 @@ __global__ void __launch_bounds__(kFinWarps * 32) finalize_kernel(const __grid_c
   const int m = blockIdx.x * kFinWarps + warp;
   __shared__ double s_sum[kFinWarps][kNacc];
   __shared__ HypState s_state[kFinWarps];
+  __shared__ PriorTerms s_prior[kFinWarps];
   if (m >= A.n_hyp || A.state[m].level != A.level) return;
+  if (A.prior_cta) {                             // what the pass kernel's prior CTA left in the workspace
+    const int* src = reinterpret_cast<const int*>(static_cast<const PriorTerms*>(A.priors) + m);
+    int* dst = reinterpret_cast<int*>(&s_prior[warp]);
+    for (int i = lane; i < (int)(sizeof(PriorTerms) / 4); i += 32) dst[i] = __ldcg(src + i);
+  }
   float t = 0.f;
   const float* p = A.partials + (size_t)m * A.n_chunks * kNacc + lane;
   for (int c = 0; c < A.n_chunks; ++c) t += __ldcg(p + (size_t)c * kNacc);      // fixed order
   s_sum[warp][lane] = (double)t;
   __syncwarp();
-  finalize_in_workspace(A, m, s_sum[warp], lane, &s_state[warp]);
+  finalize_in_workspace(A, m, s_sum[warp], lane, &s_state[warp], A.prior_cta ? &s_prior[warp] : nullptr);
 }
 
 __global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init,
@@ -151,7 +157,7 @@ bool shape_supported(const pilot_refine_config* c) {
   return true;
 }
 
-struct WsLayout { size_t state, counters, partials, scratch, total; int max_chunks; };
+struct WsLayout { size_t state, counters, priors, partials, scratch, total; int max_chunks; };
 
 WsLayout ws_layout(const pilot_refine_config* c) {
   WsLayout w;
@@ -159,6 +165,7 @@ WsLayout ws_layout(const pilot_refine_config* c) {
   size_t o = 0;
   w.state = o;    o = align_up(o + sizeof(HypState) * (size_t)c->max_hypotheses, 256);
   w.counters = o; o = align_up(o + sizeof(unsigned) * (size_t)c->max_hypotheses, 256);
+  w.priors = o;   o = align_up(o + sizeof(PriorTerms) * (size_t)c->max_hypotheses, 256);   // deferred finalisation: the prior CTAs' terms
   w.partials = o; o = align_up(o + sizeof(float) * kNacc * (size_t)c->max_hypotheses * (size_t)w.max_chunks, 256);
   w.scratch = o;  o = align_up(o + 256, 256);
   w.total = o;
@@ -417,6 +424,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
   A.n_hyp = in->n_hypotheses; A.level_end = level_end;
   A.state = reinterpret_cast<HypState*>(h->ws + w.state);
   A.counters = reinterpret_cast<unsigned*>(h->ws + w.counters);
+  A.priors = h->ws + w.priors;
   A.partials = reinterpret_cast<float*>(h->ws + w.partials);
   A.out = *out;
   A.iter_poses = h->iter_poses; A.iter_accept = h->iter_accept;
@@ -460,13 +468,18 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
         if (prev != c.device) cudaSetDevice(prev);
         return PILOT_ERR_CUDA;
       }
-      dim3 grid((unsigned)A.n_hyp, (unsigned)A.n_chunks);
+      const bool range_on = p->range_mode != PILOT_RANGE_OFF && p->w_range > 0.f && in->dsm_dev != nullptr;
       // small CTAs (<= 512 anchors) in more than one wave, or many hypotheses (measured: config 2, H = 1024, 7.01 -> 6.76 ms;
       // config 4, H = 256, 7.01 -> 6.97): the serial tail moves to its own launch
       const int per_cta = A.chunk < L.N ? A.chunk : L.N;
       A.defer = h->mode == PILOT_EXEC_PASSES_SPLIT ||
                 (h->mode == PILOT_EXEC_AUTO &&
                  ((per_cta <= 512 && (long)A.n_hyp * A.n_chunks > 2L * h->sm_count) || A.n_hyp >= 256));
+      // the prior CTAs (pilot_pass.cuh) pay when the range prior marches the heightfield and a hypothesis has many gather
+      // CTAs to hide them behind: config 4 (43 chunks) 6.97 -> 6.93 ms; with 6 chunks (config 2) the extra row of mostly empty
+      // CTAs costs more than the march it hides (6.76 -> 6.80), and the HEIGHT mode has no march to hide
+      A.prior_cta = (A.defer && range_on && p->range_mode == PILOT_RANGE_MARCH && A.n_chunks >= 16) ? 1 : 0;
+      dim3 grid((unsigned)A.n_hyp, (unsigned)(A.n_chunks + A.prior_cta));
       for (int pass = 0; pass <= p->iters[l]; ++pass) {
         A.pass = pass;
         if (mma) {
@@ -483,7 +496,7 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
           ++launches;
         }
       }
-      A.defer = 0;
+      A.defer = 0; A.prior_cta = 0;
     }
     rec_base += p->iters[l];
   }
