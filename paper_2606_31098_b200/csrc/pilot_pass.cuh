@@ -8,6 +8,7 @@ namespace {
 
 template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) photo_pass_kernel(const __grid_constant__ PassArgs A) {
+  pdl_prologue();
   const int m = blockIdx.x;
   int chunk_idx = blockIdx.y;
   const HypState* st = A.state + m;

@@ -51,6 +51,6 @@ int pilot_internal::mma_pass_launch(pilot_dtype dtype, int lanes_per_unit, const
   if (smem > 48 * 1024 - 2 * 1024 &&
       cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return (int)cudaErrorInvalidValue;
-  fn<<<dim3((unsigned)A.n_hyp, (unsigned)(A.n_chunks + A.prior_cta)), kThreads, smem, static_cast<cudaStream_t>(stream)>>>(A);
-  return (int)cudaGetLastError();
+  return (int)launch_pdl(fn, dim3((unsigned)A.n_hyp, (unsigned)(A.n_chunks + A.prior_cta)), kThreads, smem,
+                         static_cast<cudaStream_t>(stream), A);
 }

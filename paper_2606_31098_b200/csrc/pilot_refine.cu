@@ -41,6 +41,7 @@ namespace {
 // need; here all hypotheses finalise side by side instead.
 constexpr int kFinWarps = 4;
 __global__ void __launch_bounds__(kFinWarps * 32) finalize_kernel(const __grid_constant__ PassArgs A) {
+  pdl_prologue();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int m = blockIdx.x * kFinWarps + warp;
   __shared__ double s_sum[kFinWarps][kNacc];
@@ -488,11 +489,11 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
             return PILOT_ERR_CUDA;
           }
         } else {
-          fn<<<grid, kThreads, smem, st>>>(A);
+          launch_pdl(fn, grid, kThreads, smem, st, A);
         }
         ++launches;
         if (A.defer) {
-          finalize_kernel<<<(A.n_hyp + kFinWarps - 1) / kFinWarps, kFinWarps * 32, 0, st>>>(A);
+          launch_pdl(finalize_kernel, dim3((unsigned)((A.n_hyp + kFinWarps - 1) / kFinWarps)), kFinWarps * 32, 0, st, A);
           ++launches;
         }
       }
