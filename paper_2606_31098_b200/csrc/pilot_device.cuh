@@ -9,6 +9,8 @@
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <math.h>
+
+#include "pilot_pdl.cuh"
 #include <stdint.h>
 #include <type_traits>
 
@@ -101,26 +103,6 @@ struct PassArgs {
 // pilot_resident.cu: one launch of the cluster-resident LM kernel for the level described by A (A.lv, A.level,
 // A.iters, A.rec_base): `cluster` CTAs per hypothesis. Returns a cudaError_t as int.
 int resident_launch(pilot_dtype dtype, int lanes_per_unit, int grad_mode, bool mma, const PassArgs& A, int cluster, void* stream);
-
-// Programmatic dependent launch of the pass strategy's kernels (pass kernel -> finalize_kernel -> next pass ...): every CTA
-// signals at its start that the NEXT kernel of the stream may be scheduled, and waits at its start for the PREVIOUS one to have
-// completed (griddepcontrol.wait also makes its memory visible), so the next kernel's CTAs are resident and waiting when the
-// last CTAs of this one finish: the launch latency between two dependent launches (22 per step of config 4, 42 of config 2)
-// leaves the critical path. Kernels launched this way MUST begin with pdl_prologue().
-__device__ __forceinline__ void pdl_prologue() {
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-}
-template <class Fn>
-inline cudaError_t launch_pdl(Fn fn, dim3 grid, unsigned threads, size_t smem, cudaStream_t st, const PassArgs& A) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = grid; cfg.blockDim = dim3(threads, 1, 1); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, fn, A);
-}
 
 // pilot_pass_mma.cu: one launch of the pass kernel with the tensor-core contraction (grid = A.n_hyp x A.n_chunks).
 int mma_pass_launch(pilot_dtype dtype, int lanes_per_unit, const PassArgs& A, void* stream);

@@ -9,6 +9,8 @@
 
 #include <cuda_runtime.h>
 #include <math.h>
+
+#include "pilot_pdl.cuh"
 #include <stdint.h>
 
 namespace {
@@ -40,6 +42,7 @@ __device__ void rodrigues(const float* w, double (&E)[9]) {
 
 __global__ void seed_kernel(const float* __restrict__ base, const float* __restrict__ off, int n, int frame,
                             float* __restrict__ out) {
+  pilot_internal::pdl_prologue();
   int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= n) return;
   double R[9], C[3], E[9];
@@ -65,6 +68,7 @@ constexpr int kSelThreads = 1024;
 __global__ void __launch_bounds__(kSelThreads) select_best_kernel(const float* __restrict__ cost,
                                                                   const float* __restrict__ poses, int n,
                                                                   int* best_idx, float* best_pose, float* best_cost) {
+  pilot_internal::pdl_prologue();
   __shared__ unsigned long long s_key[kSelThreads / 32];
   unsigned long long k = ~0ull;
   for (int i = threadIdx.x; i < n; i += kSelThreads) {
@@ -96,6 +100,7 @@ __global__ void __launch_bounds__(kSelThreads) select_best_kernel(const float* _
 __global__ void __launch_bounds__(kSelThreads) topk_kernel(const float* __restrict__ cost,
                                                            const float* __restrict__ poses, int n, int k, int n_pow2,
                                                            int* idx_out, float* poses_out, float* cost_out) {
+  pilot_internal::pdl_prologue();
   extern __shared__ unsigned long long s[];
   for (int i = threadIdx.x; i < n_pow2; i += kSelThreads) s[i] = i < n ? make_key(cost[i], i) : ~0ull;
   __syncthreads();
@@ -157,17 +162,15 @@ int pilot_refine_seed_hypotheses(const float* base_pose_dev, const float* offset
   if (n < 0 || (frame != PILOT_SEED_CAMERA && frame != PILOT_SEED_WORLD)) return PILOT_ERR_ARG;
   if (n == 0) return PILOT_OK;
   if (!base_pose_dev || !offsets_dev || !out_poses_dev) return PILOT_ERR_ARG;
-  seed_kernel<<<(n + 127) / 128, 128, 0, static_cast<cudaStream_t>(cuda_stream)>>>(base_pose_dev, offsets_dev, n, frame,
-                                                                                    out_poses_dev);
-  return cudaGetLastError() == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
+  return pilot_internal::launch_pdl(seed_kernel, dim3((unsigned)((n + 127) / 128)), 128, 0, static_cast<cudaStream_t>(cuda_stream),
+                                    base_pose_dev, offsets_dev, n, frame, out_poses_dev) == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
 }
 
 int pilot_refine_select_best(const float* cost_dev, const float* poses_dev, int n, int* best_idx_dev,
                              float* best_pose_dev, float* best_cost_dev, void* cuda_stream) {
   if (n < 1 || !cost_dev || (best_pose_dev && !poses_dev)) return PILOT_ERR_ARG;
-  select_best_kernel<<<1, kSelThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(cost_dev, poses_dev, n, best_idx_dev,
-                                                                                     best_pose_dev, best_cost_dev);
-  return cudaGetLastError() == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
+  return pilot_internal::launch_pdl(select_best_kernel, dim3(1), kSelThreads, 0, static_cast<cudaStream_t>(cuda_stream), cost_dev, poses_dev,
+                                    n, best_idx_dev, best_pose_dev, best_cost_dev) == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
 }
 
 int pilot_refine_prune_topk(const float* cost_dev, const float* poses_dev, int n, int k, int* idx_out_dev,
@@ -180,9 +183,8 @@ int pilot_refine_prune_topk(const float* cost_dev, const float* poses_dev, int n
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return PILOT_ERR_CUDA;
-  topk_kernel<<<1, kSelThreads, smem, static_cast<cudaStream_t>(cuda_stream)>>>(cost_dev, poses_dev, n, k, n_pow2,
-                                                                               idx_out_dev, poses_out_dev, cost_out_dev);
-  return cudaGetLastError() == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
+  return pilot_internal::launch_pdl(topk_kernel, dim3(1), kSelThreads, smem, static_cast<cudaStream_t>(cuda_stream), cost_dev, poses_dev, n, k,
+                                    n_pow2, idx_out_dev, poses_out_dev, cost_out_dev) == cudaSuccess ? PILOT_OK : PILOT_ERR_CUDA;
 }
 
 }  // extern "C"

@@ -63,6 +63,7 @@ __global__ void __launch_bounds__(kFinWarps * 32) finalize_kernel(const __grid_c
 
 __global__ void init_state_kernel(HypState* state, unsigned* counters, const float* poses, int n_hyp, double lambda_init,
                                   int level_begin) {
+  pdl_prologue();
   int m = blockIdx.x * blockDim.x + threadIdx.x;
   if (m >= n_hyp) return;
   HypState s;
@@ -432,8 +433,8 @@ int pilot_refine_run_levels(pilot_refine_handle* h, const pilot_refine_inputs* i
 
   int launches = 0;
   unsigned plan_mma = 0u, plan_res = 0u;
-  init_state_kernel<<<(A.n_hyp + 127) / 128, 128, 0, st>>>(A.state, A.counters, in->init_poses_dev, A.n_hyp, (double)p->lambda_init,
-                                                                  level_begin);
+  launch_pdl(init_state_kernel, dim3((unsigned)((A.n_hyp + 127) / 128)), 128, 0, st, A.state, A.counters, in->init_poses_dev, A.n_hyp,
+             (double)p->lambda_init, level_begin);
   ++launches;
   int rec_base = 0;
   for (int l = 0; l < level_end; ++l) {

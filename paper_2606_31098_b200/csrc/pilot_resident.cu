@@ -95,6 +95,7 @@ __device__ __forceinline__ void stage_pose(ResidentShared& sh, int lane, int lev
 
 template <class T, int G, bool CEN, bool MMA>
 __global__ void __launch_bounds__(kThreads, PILOT_MIN_BLOCKS) lm_resident_kernel(const __grid_constant__ PassArgs A) {
+  pdl_prologue();
   cg::cluster_group cluster = cg::this_cluster();
   const unsigned S = cluster.num_blocks(), rank = cluster.block_rank();
   const int m = (int)(blockIdx.x / S);
@@ -249,12 +250,14 @@ int pilot_internal::resident_launch(pilot_dtype dtype, int lanes_per_unit, int g
     return (int)cudaErrorInvalidValue;
   cfg.dynamicSmemBytes = smem;
   cfg.stream = static_cast<cudaStream_t>(stream);
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = (unsigned)cluster;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see pdl_prologue (pilot_device.cuh)
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   return (int)cudaLaunchKernelEx(&cfg, fn, A);
 }
